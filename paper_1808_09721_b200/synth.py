@@ -1,0 +1,142 @@
+"""Seeded synthetic inputs for the five BASELINE.json configs.
+
+This module serves BOTH the CUDA path and the CPU oracle and therefore holds none of the
+method's arithmetic: it only writes down initial *primitive* fields (rho, v, p, B, E) and
+the run parameters.  prim->cons, Gauss's law, con2prim etc. are done by whichever side
+consumes the arrays.  The paper measures on its own initial data (Brio-Wu, KHI; PAPER.md
+L260-354), not on a public suite; these configs are synthetic stand-ins with those shapes.
+
+Arrays: float64, variable-major SoA, interior cells only, ``prims[var, k, j, i]`` (x fastest).
+Resistive prims (11): rho, vx, vy, vz, p, Bx, By, Bz, Ex, Ey, Ez.
+Two-fluid prims (16): rho_e, v_e(3), p_e, rho_p, v_p(3), p_p, B(3), E(3).
+"""
+import numpy as np
+
+RESISTIVE, TWO_FLUID = 0, 1
+BC_OUTFLOW, BC_PERIODIC = 0, 1
+
+SSP2_GAMMA = 1.0 - 1.0 / np.sqrt(2.0)
+
+
+def cell_centres(n, lo, hi):
+    dx = (hi - lo) / n
+    return lo + (np.arange(n) + 0.5) * dx
+
+
+def _minus_v_cross_B(v, B):
+    """E = -v x B (ideal-MHD initial electric field; initial data, not the scheme)."""
+    return -np.stack([v[1] * B[2] - v[2] * B[1], v[2] * B[0] - v[0] * B[2], v[0] * B[1] - v[1] * B[0]])
+
+
+def config1(nx=128):
+    """1D resistive Riemann tube (BASELINE.json configs[0]); 128 steps at nx=128 reach t=0.4."""
+    x = cell_centres(nx, -0.5, 0.5)
+    left = x < 0.0
+    w = np.zeros((11, 1, 1, nx))
+    w[0, 0, 0] = np.where(left, 1.0, 0.125)
+    w[4, 0, 0] = np.where(left, 1.0, 0.1)
+    w[5, 0, 0] = 0.5
+    w[6, 0, 0] = np.where(left, 1.0, -1.0)
+    params = dict(model=RESISTIVE, nx=nx, ny=1, nz=1, ng=4, xlim=(-0.5, 0.5), ylim=(0.0, 1.0), zlim=(0.0, 1.0),
+                  bc=(BC_OUTFLOW,) * 3, gamma=2.0, sigma=1e4, kappa=1.0, cfl=0.4)
+    return dict(name="cfg1_tube", params=params, prims=w, rho_charge=None, nsteps=nx, tol=1e-9)
+
+
+def config2(ncells=2 ** 20, seed=0):
+    """Batched implicit-stage microbench (BASELINE.json configs[1]): independent resistive cells."""
+    rng = np.random.default_rng(seed)
+    rho = 10.0 ** rng.uniform(-1.0, 1.0, ncells)
+    p = 10.0 ** rng.uniform(-2.0, 1.0, ncells)
+    dirs = rng.standard_normal((3, ncells))
+    dirs /= np.sqrt((dirs ** 2).sum(axis=0))
+    v = dirs * (0.9 * rng.uniform(0.0, 1.0, ncells) ** (1.0 / 3.0))
+    B = rng.standard_normal((3, ncells))
+    E = _minus_v_cross_B(v, B) + 0.01 * rng.standard_normal((3, ncells))
+    sigma = 10.0 ** rng.uniform(0.0, 6.0, ncells)
+    w = np.concatenate([rho[None], v, p[None], B, E], axis=0)
+    params = dict(model=RESISTIVE, nx=1, ny=1, nz=1, ng=4, gamma=4.0 / 3.0, sigma=1.0, kappa=1.0, cfl=0.4)
+    return dict(name="cfg2_stage_batch", params=params, prims=np.ascontiguousarray(w), sigma_cell=sigma,
+                a_dt=SSP2_GAMMA * 1e-3, tol=1e-10)
+
+
+def config3(nx=512, ny=512, nsteps=200):
+    """2D resistive shear layer (BASELINE.json configs[2]); periodic x / outflow y."""
+    x = cell_centres(nx, -0.5, 0.5)[None, :]
+    y = cell_centres(ny, -1.0, 1.0)[:, None]
+    w = np.zeros((11, 1, ny, nx))
+    w[0] = 1.0
+    w[4] = 1.0
+    vx = 0.5 * np.tanh(y / 0.01) + 0.0 * x
+    vy = 0.1 * np.sin(2.0 * np.pi * x) * np.exp(-y ** 2 / 0.01)
+    w[1, 0], w[2, 0] = vx, vy
+    w[7] = 0.1
+    w[8:11] = _minus_v_cross_B(w[1:4], w[5:8])
+    params = dict(model=RESISTIVE, nx=nx, ny=ny, nz=1, ng=4, xlim=(-0.5, 0.5), ylim=(-1.0, 1.0), zlim=(0.0, 1.0),
+                  bc=(BC_PERIODIC, BC_OUTFLOW, BC_OUTFLOW), gamma=4.0 / 3.0, sigma=1e3, kappa=1.0, cfl=0.4)
+    return dict(name="cfg3_shear", params=params, prims=w, rho_charge=None, nsteps=nsteps, tol=1e-8)
+
+
+def config4(nx=1024, ny=1024, nsteps=50, seed=0):
+    """2D two-fluid pair plasma with seeded smooth velocity (BASELINE.json configs[3]); periodic."""
+    rng = np.random.default_rng(seed)
+    A = rng.uniform(-1.0, 1.0, (2, 4))
+    th = rng.uniform(0.0, 2.0 * np.pi, (2, 4))
+    kvec = [(1, 0), (0, 1), (1, 1), (1, -1)]
+    x = cell_centres(nx, 0.0, 1.0)[None, :]
+    y = cell_centres(ny, 0.0, 1.0)[:, None]
+    v = np.zeros((3, 1, ny, nx))
+    for c in range(2):
+        for m, (kx, ky) in enumerate(kvec):
+            v[c, 0] += A[c, m] * np.sin(2.0 * np.pi * (kx * x + ky * y) + th[c, m])
+    v *= 0.4 / np.sqrt((v ** 2).sum(axis=0)).max()
+    w = np.zeros((16, 1, ny, nx))
+    for s in range(2):
+        w[5 * s + 0] = 0.5
+        w[5 * s + 1:5 * s + 4] = v
+        w[5 * s + 4] = 0.5
+    w[10] = 0.2
+    w[13:16] = _minus_v_cross_B(v, w[10:13])
+    params = dict(model=TWO_FLUID, nx=nx, ny=ny, nz=1, ng=4, xlim=(0.0, 1.0), ylim=(0.0, 1.0), zlim=(0.0, 1.0),
+                  bc=(BC_PERIODIC,) * 3, gamma=4.0 / 3.0, eta=1e-4, mu_e=-100.0, mu_p=100.0, kappa=1.0, cfl=0.4)
+    return dict(name="cfg4_two_fluid", params=params, prims=w, rho_charge=None, nsteps=nsteps, tol=1e-8)
+
+
+def config5(n=256, nsteps=20):
+    """3D resistive blast (BASELINE.json configs[4]); outflow."""
+    c = cell_centres(n, -0.5, 0.5)
+    r2 = c[:, None, None] ** 2 + c[None, :, None] ** 2 + c[None, None, :] ** 2
+    w = np.zeros((11, n, n, n))
+    w[0] = 1.0
+    w[4] = np.where(r2 < 0.1 ** 2, 1.0, 0.01)
+    w[5] = 0.1
+    params = dict(model=RESISTIVE, nx=n, ny=n, nz=n, ng=4, xlim=(-0.5, 0.5), ylim=(-0.5, 0.5), zlim=(-0.5, 0.5),
+                  bc=(BC_OUTFLOW,) * 3, gamma=4.0 / 3.0, sigma=1e5, kappa=1.0, cfl=0.3)
+    return dict(name="cfg5_blast", params=params, prims=w, rho_charge=None, nsteps=nsteps, tol=1e-8)
+
+
+def random_resistive_prims(n, seed, vmax=0.99, with_E=True):
+    """Random admissible resistive primitive states (round-trip pins, kernel unit tests)."""
+    rng = np.random.default_rng(seed)
+    rho = 10.0 ** rng.uniform(-2.0, 2.0, n)
+    p = 10.0 ** rng.uniform(-3.0, 2.0, n)
+    dirs = rng.standard_normal((3, n))
+    dirs /= np.sqrt((dirs ** 2).sum(axis=0))
+    v = dirs * (vmax * rng.uniform(0.0, 1.0, n))
+    B = rng.standard_normal((3, n))
+    E = rng.standard_normal((3, n)) if with_E else np.zeros((3, n))
+    return np.ascontiguousarray(np.concatenate([rho[None], v, p[None], B, E], axis=0))
+
+
+def random_two_fluid_prims(n, seed, vmax=0.9):
+    rng = np.random.default_rng(seed)
+    parts = []
+    for _ in range(2):
+        rho = 10.0 ** rng.uniform(-1.0, 1.0, n)
+        p = 10.0 ** rng.uniform(-2.0, 1.0, n)
+        dirs = rng.standard_normal((3, n))
+        dirs /= np.sqrt((dirs ** 2).sum(axis=0))
+        v = dirs * (vmax * rng.uniform(0.0, 1.0, n))
+        parts += [rho[None], v, p[None]]
+    B = rng.standard_normal((3, n))
+    E = rng.standard_normal((3, n))
+    return np.ascontiguousarray(np.concatenate(parts + [B, E], axis=0))
