@@ -1,0 +1,334 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of one full IMEX SSP2(222) step (all SURVEY.md 8(a) rows) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg5|cfg2|...]
+
+Workload at N=1: BASELINE.json configs[4], the 3-D 256^3 resistive blast -- the configuration
+the metric ("FP64 zone-updates/s per full IMEX step") and the north-star target are quoted on;
+configs[1] is a single implicit stage, not a full step, so it is a parity case and an optional
+`--workload cfg2` line, not the headline.  Inputs are synthetic (paper_1808_09721_b200.synth).
+Prints ONE JSON line (rank 0).  Multi-GPU: the path does not shard in this build ("replicas
+only"): each rank steps its own copy; value = zone-updates of all ranks / max time.
+
+`--impl reference` times the CPU oracle as it stands on the host cores, on a bounded sample of
+the same workload (a 64^3 sub-box of the 256^3 initial data around the blast, one step per
+"step").  The oracle is a deliberately slow checker: the ratio to it is context, not a target.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fp64_zone_updates_per_s_full_imex_step"
+UNIT = "zone-updates/s"
+SM_COUNT = 148
+FP64_LANES_PER_SM = 64          # FP64 FMA lanes per SM (B200_PROFILING.md has no FP64 figure; DESIGN.md derives it)
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return d.get("hbm_gbs", 6650.0), d.get("sm_max_mhz", 1965.0), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+# ---- clocks during the timed region ----------------------------------------------------------
+class ClockSampler:
+    def __init__(self, index=0, period=0.02):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._t = None
+        self.index, self.period = index, period
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def _reason_names(self, mask):
+        nv = self.nv
+        table = {
+            "hw_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8),
+            "hw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40),
+            "sw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20),
+            "sw_power_cap": getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4),
+            "hw_power_brake": getattr(nv, "nvmlClocksThrottleReasonHwPowerBrakeSlowdown", 0x80),
+        }
+        return {k for k, bit in table.items() if mask & bit}
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                self.reasons |= self._reason_names(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def __enter__(self):
+        if self.nv:
+            self._t = threading.Thread(target=self._run, daemon=True)
+            self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._t:
+            self._t.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["unavailable"]}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+# ---- workloads ---------------------------------------------------------------------------------
+def make_workload(name, synth):
+    if name == "cfg5":
+        return synth.config5()
+    if name == "cfg3":
+        return synth.config3()
+    if name == "cfg1":
+        return synth.config1()
+    if name == "cfg5_small":
+        return synth.config5(n=64)
+    raise SystemExit(f"unknown workload {name}")
+
+
+def oracle_sample(cfg, synth):
+    """A bounded sample of the workload for the CPU oracle: central 64^3 (or whole grid if smaller)."""
+    p = dict(cfg["params"])
+    w = cfg["prims"]
+    nz, ny, nx = w.shape[1:]
+    m = 64
+    if nz > m and ny > m and nx > m:
+        sl = [slice((n - m) // 2, (n - m) // 2 + m) for n in (nz, ny, nx)]
+        dx = [(p["zlim"][1] - p["zlim"][0]) / nz, (p["ylim"][1] - p["ylim"][0]) / ny, (p["xlim"][1] - p["xlim"][0]) / nx]
+        lim = lambda lo, s, d: (lo + s.start * d, lo + s.stop * d)
+        p.update(nx=m, ny=m, nz=m, zlim=lim(p["zlim"][0], sl[0], dx[0]), ylim=lim(p["ylim"][0], sl[1], dx[1]),
+                 xlim=lim(p["xlim"][0], sl[2], dx[2]))
+        w = np.ascontiguousarray(w[:, sl[0], sl[1], sl[2]])
+        what = f"central {m}^3 sub-box of the {nx}^3 initial data (same dx), 1 oracle step per sample step"
+    else:
+        what = "the whole grid, 1 oracle step per sample step"
+    return p, w, what
+
+
+def time_oracle(cfg, synth, steps, warmup, budget_s=40.0):
+    from oracle import oracle as O
+    p, w, what = oracle_sample(cfg, synth)
+    cores = O.set_threads(0)
+    S = O.OracleSim(O.make_params(**p))
+    S.set_initial(w, cfg.get("rho_charge"))
+    ncell = w.shape[1] * w.shape[2] * w.shape[3]
+    t0 = time.perf_counter()
+    for _ in range(max(warmup, 0)):
+        S.step(1)
+        if time.perf_counter() - t0 > budget_s / 2:
+            break
+    t0 = time.perf_counter()
+    done = 0
+    for _ in range(steps):
+        S.step(1)
+        done += 1
+        if time.perf_counter() - t0 > budget_s:
+            break
+    dt = time.perf_counter() - t0
+    S.close()
+    return {"value": ncell * done / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{what}; {done} steps in {dt:.1f} s"}, dt / done * 1e3, done
+
+
+# ---- reference arm --------------------------------------------------------------------------
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_1808_09721_b200 import synth
+    cfg = make_workload(args.workload, synth)
+    base, ms, done = time_oracle(cfg, synth, args.steps, min(args.warmup, 1), budget_s=120.0)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": base["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": done,
+        "warmup": min(args.warmup, 1), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg["name"] + " (oracle sample)", "sample": base["sample"]},
+        "cpu_baseline": base,
+        "e2e": {"value": base["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# ---- our arm ----------------------------------------------------------------------------------
+def stage_flops(hist):
+    """Algorithmic flops of one resistive implicit-stage launch from the logged iteration histogram.
+    Per Newton iteration of the 4x4 system (stage.cuh r_stage_iter; FMA = 2, div/rsqrt = 1):
+    ~420 flop; init + finish ~150 flop."""
+    its = (hist * np.arange(hist.size)).sum()
+    n = hist.sum()
+    return 420.0 * its + 150.0 * n
+
+
+def run_ours(args):
+    import torch
+    from paper_1808_09721_b200 import binding as B, synth
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    B.lib()
+    hbm_peak, sm_max_mhz, peak_src = load_peaks()
+    dev = torch.device("cuda", local)
+
+    cfg = make_workload(args.workload, synth)
+    p = dict(cfg["params"]); p["device"] = local
+    nz, ny, nx = cfg["prims"].shape[1:]
+    ncell = nx * ny * nz
+    sim = B.Rmhd(**p)
+    prims_d = torch.from_numpy(np.ascontiguousarray(cfg["prims"])).to(dev)
+    sim.set_initial(prims_d)
+    del prims_d
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing -------------------------------------------------------------
+    for _ in range(args.warmup):
+        sim.step(1)
+    B.rmhd_set_profiling(sim.ctx, True)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    with ClockSampler(local) as clk:
+        ev0.record()
+        for _ in range(args.steps):
+            sim.step(1)
+        ev1.record()
+        barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    kt = B.rmhd_get_kernel_times(sim.ctx)
+    stats = sim.stats()
+    B.rmhd_set_profiling(sim.ctx, False)
+    t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total = float(t.item())
+    value = world * ncell * args.steps / (ms_total * 1e-3)
+
+    # ---- roofline of the dominant kernel class -------------------------------------------------
+    naxes = sum(1 for n in (nx, ny, nz) if n > 1)
+    dom = max(("stage1", "stage2", "flux", "combine_c2p"), key=lambda k: kt[k]["ms"])
+    avg_ms = kt[dom]["ms"] / max(kt[dom]["launches"], 1)
+    shares = {k: round(v["ms"] / max(sum(x["ms"] for x in kt.values()), 1e-30), 4) for k, v in kt.items()}
+    alg_bytes = {  # SURVEY.md 8(d) table, doubles per cell per launch x 8 B (resistive)
+        "stage1": 29 * 8 * ncell, "stage2": 57 * 8 * ncell, "flux": 33 * 8 * ncell / max(naxes, 1),
+        "combine_c2p": 76 * 8 * ncell,   # 76 incl. the fused F2 reads; the un-fused kernel's own minimum is 62
+    }
+    if dom in ("stage1", "stage2"):
+        nsolve = stats["hist_stage"].sum()
+        fl = stage_flops(stats["hist_stage"]) / max(nsolve, 1) * ncell
+        peak_tf = SM_COUNT * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 * 1e-12
+        roof = {"bound": "alu", "kernel": dom, "achieved": fl / (avg_ms * 1e-3) * 1e-12, "peak": peak_tf, "unit": "TFLOP/s",
+                "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x sm_max_mhz (DESIGN.md)", "traffic": None}
+    else:
+        roof = {"bound": "hbm", "kernel": dom, "achieved": alg_bytes[dom] / (avg_ms * 1e-3) * 1e-9, "peak": hbm_peak,
+                "unit": "GB/s", "peak_source": peak_src + " (MEASURED_PEAKS.json hbm_gbs)", "traffic": None}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof["avg_launch_ms"] = avg_ms
+    roof["kernel_time_shares"] = shares
+    step_alg_bytes = 195 * 8 * ncell
+    roof["whole_step_hbm_frac"] = step_alg_bytes / (ms_total / args.steps * 1e-3) * 1e-9 / hbm_peak
+
+    # ---- end to end through the C-ABI with host buffers ---------------------------------------
+    e2e = None
+    if rank == 0 or world > 1:
+        nc, npr = B.NCONS[p["model"]], B.NPRIM[p["model"]]
+        cons_h = torch.empty((nc, nz, ny, nx), dtype=torch.float64, pin_memory=True)
+        prims_h = torch.empty((npr, nz, ny, nx), dtype=torch.float64, pin_memory=True)
+        B.rmhd_get_state(sim.ctx, cons_h, prims_h)
+        e_steps = max(1, min(args.steps, 3))
+        barrier()
+        ev0.record()
+        for _ in range(e_steps):
+            B.rmhd_set_cons(sim.ctx, cons_h, prims_h)      # H2D of this step's input state (+ guess)
+            sim.step(1)
+            B.rmhd_get_state(sim.ctx, cons_h, prims_h)     # D2H of the step's result
+        ev1.record()
+        barrier()
+        t = torch.tensor([ev0.elapsed_time(ev1)], dtype=torch.float64, device=dev)
+        if dist is not None:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        nh = 5 if p["model"] == 0 else 10
+        e2e = {"value": world * ncell * e_steps / (float(t.item()) * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": (nc + nh) * ncell * 8, "d2h_bytes_per_step": (nc + npr) * ncell * 8,
+               "steps": e_steps, "call": "rmhd_set_cons(host) + rmhd_step(1) + rmhd_get_state(host), pinned host buffers"}
+        del cons_h, prims_h
+    n_failed = stats["n_failed"]
+    sim.close()
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+    cpu_base = None
+    if world == 1 and not args.no_cpu_baseline:
+        cpu_base, _, _ = time_oracle(cfg, synth, steps=2, warmup=0, budget_s=30.0)
+    launches = sum(v["launches"] for v in kt.values())
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{cfg['name']}: {nx}x{ny}x{nz} cells, {'resistive' if p['model'] == 0 else 'two_fluid'}, "
+                               f"SSP2(222), cfl {p['cfl']}, sigma {p.get('sigma')}",
+                   "parallelism": "replicas only" if world > 1 else "1 gpu",
+                   "l2": "state arrays (%.1f GB) exceed the 126 MB L2; no flush needed" % (71 * ncell * 8 / 1e9),
+                   "n_failed_cells": int(n_failed),
+                   "stage_iters_mean": float((stats["hist_stage"] * np.arange(stats["hist_stage"].size)).sum() / max(stats["hist_stage"].sum(), 1))},
+        "clocks": clk.summary(), "e2e": e2e, "gpu_launches": int(launches),
+        "roofline": roof, "cpu_baseline": cpu_base,
+    }
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg5")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

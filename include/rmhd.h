@@ -1,0 +1,141 @@
+/* =====================================================================================
+ * rmhd.h -- C-ABI of librmhd.so: one GPU, FP64, finite-volume IMEX SSP2(222) step for
+ * special-relativistic resistive MHD (14 conserved variables) and two-fluid RMHD (18)
+ * after Wright & Hawke, "Resistive and multi-fluid RMHD on graphics processing units"
+ * (citations "P:Lnnn" are line numbers of the reference text PAPER.md; "Gn" are the
+ * readings listed in DESIGN.md).
+ *
+ * Plain pointers and sizes only; no torch types.  Every entry point returns 0 on success or
+ * a negative RMHD_ERR_* code; nothing throws or aborts across the boundary.  There is no CPU
+ * fallback: without a CUDA device rmhd_create / the *_batch calls return RMHD_ERR_CUDA.
+ *
+ * ARRAY LAYOUT at the boundary (all double): interior cells only, variable-major SoA,
+ *   grids   a[var][k][j][i]  (i = x fastest),   batches  a[var][cell].
+ *   resistive cons  (14): D, Sx,Sy,Sz, tau, Bx,By,Bz, Ex,Ey,Ez, rho_charge, psi, phi (eq 1)
+ *   resistive prims (11): rho, vx,vy,vz, p, Bx,By,Bz, Ex,Ey,Ez
+ *   two-fluid cons  (18): D, S(3), tau, Dbar, Sbar(3), taubar, B(3), E(3), psi, phi   (eq 5-6)
+ *   two-fluid prims (16): rho_e, v_e(3), p_e, rho_p, v_p(3), p_p, B(3), E(3)
+ * OWNERSHIP: the caller owns every buffer it passes (host or device as flagged by
+ * `on_device`; device buffers must live on the context's device); the library owns the
+ * context and all its internal device state, released by rmhd_destroy.
+ * ===================================================================================== */
+#ifndef RMHD_H
+#define RMHD_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rmhd_ctx rmhd_ctx; /* opaque */
+
+enum { RMHD_RESISTIVE = 0, RMHD_TWO_FLUID = 1 };
+enum { RMHD_BC_OUTFLOW = 0, RMHD_BC_PERIODIC = 1 };
+enum {
+  RMHD_OK = 0,
+  RMHD_ERR_BAD_PARAM = -1,
+  RMHD_ERR_CUDA = -2,
+  RMHD_ERR_NONCONVERGED = -3,   /* some cell's root-find failed; state still advanced */
+  RMHD_ERR_UNPHYSICAL_INPUT = -4
+};
+
+/* Statement of the problem as the paper gives it: model, Gamma-law EOS, sigma or
+ * (eta, mu_s), kappa, grid, CFL, boundary conditions. */
+typedef struct {
+  int model;                  /* RMHD_RESISTIVE | RMHD_TWO_FLUID                                */
+  int nx, ny, nz;             /* interior cells; n == 1 => that axis is absent                  */
+  int ng;                     /* ghost layers of the paper's layout (>= 2).  Ghost zones are     */
+                              /* virtual here (boundary index maps inside the stencil loads), so */
+                              /* ng only has to be >= the stencil reach; kept for API parity     */
+  double xmin, xmax, ymin, ymax, zmin, zmax;
+  int bc[3];                  /* per axis: RMHD_BC_OUTFLOW (zero gradient) | RMHD_BC_PERIODIC    */
+  double gamma;               /* Gamma-law index                                                 */
+  double sigma;               /* resistive: conductivity                                         */
+  double eta, mu_e, mu_p;     /* two-fluid: resistivity, charge/mass ratios (mu_e != mu_p)        */
+  double kappa;               /* divergence-cleaning rate; the paper uses 1              */
+  double cfl;                 /* dt = cfl / sum_d (1/dx_d) over present axes, fixed (G9)          */
+  double tol_c2p, tol_stage;  /* relative Newton-update tolerances; <= 0 => 1e-13, 1e-12 */
+  int max_iter_c2p, max_iter_stage; /* <= 0 => 100, 50                                          */
+  int device;                 /* CUDA ordinal                                                    */
+  void* stream;               /* cudaStream_t owned by the caller (0 = default stream)           */
+} rmhd_params;
+
+/* ---- grid simulation (north_star: rmhd_create / set_initial / step / get_state / destroy) -- */
+
+/* Allocate all device state for one grid.  Errors: BAD_PARAM (sizes, ng < 2, mu_e == mu_p,
+ * gamma <= 1), CUDA (no device / out of memory). */
+int rmhd_create(const rmhd_params* p, rmhd_ctx** out);
+
+/* Initial primitives -> conserved state (eq 2-4; eq 6), psi = phi = 0
+ * (P:L81).  prims: [11|16][nz][ny][nx].  rho_charge: [nz][ny][nx] or NULL => Gauss's law
+ * rho = div E by 2nd-order central differences with the boundary conditions applied
+ * (G10); ignored for the two-fluid model (charge density is Dbar).  Resets time and
+ * statistics.  Errors: UNPHYSICAL_INPUT if any cell has rho <= 0, p <= 0 or |v| >= 1. */
+int rmhd_set_initial(rmhd_ctx* c, const double* prims, const double* rho_charge, int on_device);
+
+/* Overwrite the conserved state (cons: [14|18][nz][ny][nx]) and recover primitives from it
+ * (P:L118-136); prim_guess nullable.  Used for restarts and by tests. */
+int rmhd_set_cons(rmhd_ctx* c, const double* cons, const double* prim_guess, int on_device);
+
+/* Advance nsteps full IMEX SSP2(222) steps (Table 2, eq 10-11 P:L152-155 read as
+ * G1): implicit stage, L(q1), implicit stage, L(q2), combine, con2prim.  Everything runs on
+ * the context's stream; one 16-byte device->host read of the failure counters at the end.
+ * Returns NONCONVERGED if any root-find failed in any cell (the steps are still completed). */
+int rmhd_step(rmhd_ctx* c, int nsteps);
+
+/* Copy out the interior state; either pointer may be NULL. */
+int rmhd_get_state(rmhd_ctx* c, double* cons, double* prims, int on_device);
+
+/* L(q) = -sum_d dF^d/dx_d of the current state: Lax-Friedrichs flux-vector
+ * splitting (eq 12, alpha = 1) + WENO3.  Lout: [14|18][nz][ny][nx].  (Unit-parity hook.) */
+int rmhd_flux_divergence(rmhd_ctx* c, double* Lout, int on_device);
+
+/* Iteration-count histograms since the last set_initial: hist_stage[b] = implicit-stage solves
+ * that took b Newton iterations, hist_c2p[b] likewise for stand-alone con2prim (last bin
+ * collects the overflow); number of failed root-finds and the smallest failing cell index
+ * (k*ny*nx + j*nx + i), -1 if none.  Any pointer may be NULL.  Host pointers. */
+int rmhd_get_stats(rmhd_ctx* c, long long* hist_stage, long long* hist_c2p, int nbins, long long* n_failed,
+                   long long* first_failed_cell);
+
+/* Per-kernel-class device time (CUDA events on the context's stream) accumulated while
+ * profiling is enabled.  Classes: 0 stage1, 1 stage2, 2 flux sweeps, 3 combine+con2prim,
+ * 4 other.  ms[n], launches[n] host arrays. */
+int rmhd_set_profiling(rmhd_ctx* c, int enabled);
+int rmhd_get_kernel_times(rmhd_ctx* c, double* ms, long long* launches, int n);
+
+double rmhd_dt(const rmhd_ctx* c);
+double rmhd_time(const rmhd_ctx* c);           /* t0 + nsteps_done * dt, never accumulated */
+const char* rmhd_last_error(const rmhd_ctx* c); /* ctx-owned string; c == NULL => last create error */
+void rmhd_destroy(rmhd_ctx* c);
+
+/* ---- batched per-cell operations on n independent cells (BASELINE.json configs[1]) --------- */
+/* Only model, gamma, sigma, eta, mu_e, mu_p, kappa, tolerances, device and stream of *p are
+ * used.  All pointers are DEVICE pointers unless on_device == 0, in which case the call
+ * stages them through temporary device buffers (host<->device copies inside the call). */
+
+/* One implicit stage (eq 10):  q* - q_ex - a_dt Psi(q*) = 0 per cell.
+ * q_ex [14|18][n]; prim_guess [11|16][n] (initial guess: primitives near the solution);
+ * sigma_cell [n] per-cell conductivity or NULL (use p->sigma; resistive only);
+ * outputs q_out [14|18][n], prims_out [11|16][n], iters [n] Newton iterations taken,
+ * fail [n] (0 ok).  iters / fail may be NULL. */
+int rmhd_stage_batch(const rmhd_params* p, long long ncells, const double* q_ex, const double* prim_guess,
+                     const double* sigma_cell, double a_dt, double* q_out, double* prims_out, int* iters,
+                     int* fail, int on_device);
+
+/* eq (2)-(4) / eq (6): prims [11|16][n] (+ rho_charge [n] or NULL = 0) -> cons [14|18][n], psi = phi = 0. */
+int rmhd_prim2cons_batch(const rmhd_params* p, long long ncells, const double* prims, const double* rho_charge,
+                         double* cons, int on_device);
+
+/* cons -> prims; prim_guess nullable; iters / fail nullable. */
+int rmhd_con2prim_batch(const rmhd_params* p, long long ncells, const double* cons, const double* prim_guess,
+                        double* prims, int* iters, int* fail, int on_device);
+
+/* ---- roofline denominators measured by the library's own probe kernels ------------------- */
+/* FP64 FMA chain on all SMs: returns achieved TFLOP/s (2 flop per DFMA) in *tflops. */
+int rmhd_probe_fp64(int device, void* stream, double* tflops);
+/* Device-to-device streaming copy of `bytes` bytes (read + write counted): GB/s. */
+int rmhd_probe_hbm(int device, void* stream, long long bytes, double* gbs);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RMHD_H */

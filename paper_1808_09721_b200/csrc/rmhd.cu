@@ -1,0 +1,569 @@
+// rmhd.cu -- C-ABI of librmhd.so (include/rmhd.h): context, launches, copies.  No CPU fallback.
+#include "rmhd.h"
+
+#include <climits>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "kernels.cuh"
+
+using namespace rmhd;
+
+namespace {
+
+enum { KC_STAGE1 = 0, KC_STAGE2 = 1, KC_FLUX = 2, KC_FINAL = 3, KC_OTHER = 4, KC_N = 5 };
+
+thread_local std::string g_create_error;
+
+struct EvRec { int cls; cudaEvent_t a, b; };
+
+}  // namespace
+
+struct rmhd_ctx {
+  rmhd_params p;
+  DevPar P;
+  int model, nc, nh, ns, np;
+  int n[3];
+  size_t N;
+  double dx[3], dt;
+  long long nsteps;
+  int device;
+  cudaStream_t stream;
+  double *q, *w, *qs, *L1, *L2, *Ps1, *Ps2;
+  Stats* d_stats;
+  Stats* h_stats;  // pinned
+  bool profiling;
+  std::vector<EvRec> pending;
+  std::vector<cudaEvent_t> ev_pool;
+  double ms[KC_N];
+  long long launches[KC_N];
+  std::string err;
+};
+
+namespace {
+
+struct DeviceGuard {
+  int prev;
+  bool ok;
+  explicit DeviceGuard(int dev) : prev(-1), ok(true) {
+    if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; prev = -1; }
+    if (cudaSetDevice(dev) != cudaSuccess) ok = false;
+  }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+int fail_cuda(rmhd_ctx* c, cudaError_t e, const char* what) {
+  char buf[256];
+  snprintf(buf, sizeof buf, "CUDA error in %s: %s", what, cudaGetErrorString(e));
+  if (c) c->err = buf; else g_create_error = buf;
+  return RMHD_ERR_CUDA;
+}
+#define CK(c, call)                                              \
+  do {                                                           \
+    cudaError_t e__ = (call);                                    \
+    if (e__ != cudaSuccess) return fail_cuda((c), e__, #call);   \
+  } while (0)
+
+int make_devpar(const rmhd_params* p, DevPar& P, std::string& err) {
+  if (p->model != RMHD_RESISTIVE && p->model != RMHD_TWO_FLUID) { err = "model must be RMHD_RESISTIVE or RMHD_TWO_FLUID"; return RMHD_ERR_BAD_PARAM; }
+  if (!(p->gamma > 1.0)) { err = "gamma must be > 1"; return RMHD_ERR_BAD_PARAM; }
+  if (p->model == RMHD_TWO_FLUID && p->mu_e == p->mu_p) { err = "mu_e must differ from mu_p"; return RMHD_ERR_BAD_PARAM; }
+  if (p->model == RMHD_RESISTIVE && !(p->sigma >= 0.0)) { err = "sigma must be >= 0"; return RMHD_ERR_BAD_PARAM; }
+  P.gam = p->gamma; P.g = (p->gamma - 1.0) / p->gamma; P.gi = p->gamma / (p->gamma - 1.0);
+  P.sigma = p->sigma; P.eta = p->eta; P.mu_e = p->mu_e; P.mu_p = p->mu_p; P.kappa = p->kappa;
+  P.tol_c2p = p->tol_c2p > 0 ? p->tol_c2p : 1e-13;
+  P.tol_stage = p->tol_stage > 0 ? p->tol_stage : 1e-12;
+  P.maxit_c2p = p->max_iter_c2p > 0 ? p->max_iter_c2p : 100;
+  P.maxit_stage = p->max_iter_stage > 0 ? p->max_iter_stage : 50;
+  return RMHD_OK;
+}
+
+inline unsigned blocks_for(size_t n, int threads) { return (unsigned)((n + threads - 1) / threads); }
+
+// ---- profiling helpers -------------------------------------------------------------------
+cudaEvent_t get_event(rmhd_ctx* c) {
+  if (!c->ev_pool.empty()) { cudaEvent_t e = c->ev_pool.back(); c->ev_pool.pop_back(); return e; }
+  cudaEvent_t e; cudaEventCreate(&e); return e;
+}
+struct Timed {
+  rmhd_ctx* c; int cls; cudaEvent_t a, b;
+  Timed(rmhd_ctx* c_, int cls_) : c(c_), cls(cls_), a(nullptr), b(nullptr) {
+    c->launches[cls]++;
+    if (c->profiling) { a = get_event(c); b = get_event(c); cudaEventRecord(a, c->stream); }
+  }
+  ~Timed() { if (c->profiling) { cudaEventRecord(b, c->stream); c->pending.push_back({cls, a, b}); } }
+};
+void resolve_events(rmhd_ctx* c) {  // stream must be synchronised
+  for (auto& r : c->pending) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, r.a, r.b) == cudaSuccess) c->ms[r.cls] += ms;
+    c->ev_pool.push_back(r.a); c->ev_pool.push_back(r.b);
+  }
+  c->pending.clear();
+}
+
+// ---- launches ----------------------------------------------------------------------------
+template <int MODEL, int AXIS>
+int launch_flux_axis(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODEL>& wr, double* L, int accumulate) {
+  constexpr int TS = Tile<AXIS>::TS, TO = Tile<AXIS>::TO;
+  static bool attr_set[8] = {false, false, false, false, false, false, false, false};
+  const size_t smem = flux_smem_bytes<MODEL, AXIS>();
+  if (!attr_set[c->device & 7]) {
+    CK(c, cudaFuncSetAttribute(k_flux<MODEL, AXIS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr_set[c->device & 7] = true;
+  }
+  const int nx = c->n[0], ny = c->n[1], nz = c->n[2];
+  const int ns = c->n[AXIS];
+  dim3 grid;
+  if (AXIS == 0) grid = dim3((ny * nz + TO - 1) / TO, (ns + TS - 1) / TS, 1);
+  else grid = dim3((nx + TO - 1) / TO, (ns + TS - 1) / TS, AXIS == 1 ? nz : ny);
+  Timed t(c, KC_FLUX);
+  k_flux<MODEL, AXIS><<<grid, FLUX_THREADS, smem, c->stream>>>(qr, wr, L, c->N, nx, ny, nz, c->p.bc[AXIS], 1.0 / c->dx[AXIS], accumulate, c->P);
+  CK(c, cudaGetLastError());
+  return RMHD_OK;
+}
+
+// L(q) with the conserved rows taken from `qa` except the rows listed in src rows, which come
+// from `qb` when mix != 0 (stage 1 only rewrites the rows that have a source).
+template <int MODEL>
+int launch_flux(rmhd_ctx* c, const double* qa, const double* qb, bool mix, const double* w, double* L) {
+  constexpr int NC = Dim<MODEL>::NC, NH = Dim<MODEL>::NH, NS = Dim<MODEL>::NS;
+  ConsRows<MODEL> qr; HydRows<MODEL> wr;
+  for (int v = 0; v < NC; ++v) qr.r[v] = qa + (size_t)v * c->N;
+  if (mix) for (int k = 0; k < NS; ++k) { int v = MODEL == 0 ? (k < 3 ? 8 + k : 9 + k) : (k < 4 ? 6 + k : 9 + k); qr.r[v] = qb + (size_t)v * c->N; }
+  for (int v = 0; v < NH; ++v) wr.r[v] = w + (size_t)v * c->N;
+  int acc = 0, rc;
+  if (c->n[0] > 1) { if ((rc = launch_flux_axis<MODEL, 0>(c, qr, wr, L, acc))) return rc; acc = 1; }
+  if (c->n[1] > 1) { if ((rc = launch_flux_axis<MODEL, 1>(c, qr, wr, L, acc))) return rc; acc = 1; }
+  if (c->n[2] > 1) { if ((rc = launch_flux_axis<MODEL, 2>(c, qr, wr, L, acc))) return rc; acc = 1; }
+  if (!acc) CK(c, cudaMemsetAsync(L, 0, sizeof(double) * NC * c->N, c->stream));
+  return RMHD_OK;
+}
+
+int step_once_resistive(rmhd_ctx* c) {
+  const double g = 1.0 - 1.0 / sqrt(2.0);
+  const double dt = c->dt;
+  const unsigned nb = blocks_for(c->N, 128);
+  int rc;
+  {
+    Timed t(c, KC_STAGE1);
+    k_stage_resistive<1><<<nb, 128, 0, c->stream>>>(c->q, nullptr, nullptr, c->w, c->qs, c->Ps1, c->N, g * dt, 0.0, 0.0, c->P, c->d_stats);
+    CK(c, cudaGetLastError());
+  }
+  if ((rc = launch_flux<0>(c, c->q, c->qs, true, c->w, c->L1))) return rc;
+  {
+    Timed t(c, KC_STAGE2);
+    k_stage_resistive<2><<<nb, 128, 0, c->stream>>>(c->q, c->L1, c->Ps1, c->w, c->qs, c->Ps2, c->N, g * dt, dt, (1.0 - 2.0 * g) * dt, c->P, c->d_stats);
+    CK(c, cudaGetLastError());
+  }
+  if ((rc = launch_flux<0>(c, c->qs, nullptr, false, c->w, c->L2))) return rc;
+  {
+    Timed t(c, KC_FINAL);
+    k_final<0><<<blocks_for(c->N, 256), 256, 0, c->stream>>>(c->q, c->L1, c->L2, c->Ps1, c->Ps2, c->w, c->N, 0.5 * dt, c->P, c->d_stats);
+    CK(c, cudaGetLastError());
+  }
+  return RMHD_OK;
+}
+
+int read_stats(rmhd_ctx* c) {
+  CK(c, cudaMemcpyAsync(c->h_stats, c->d_stats, sizeof(Stats), cudaMemcpyDeviceToHost, c->stream));
+  CK(c, cudaStreamSynchronize(c->stream));
+  resolve_events(c);
+  return RMHD_OK;
+}
+
+int reset_stats(rmhd_ctx* c) {
+  memset(c->h_stats, 0, sizeof(Stats));
+  c->h_stats->first_failed = LLONG_MAX;
+  CK(c, cudaMemcpyAsync(c->d_stats, c->h_stats, sizeof(Stats), cudaMemcpyHostToDevice, c->stream));
+  return RMHD_OK;
+}
+
+}  // namespace
+
+// =========================================================================================
+extern "C" {
+
+int rmhd_create(const rmhd_params* p, rmhd_ctx** out) {
+  if (!p || !out) { g_create_error = "null argument"; return RMHD_ERR_BAD_PARAM; }
+  *out = nullptr;
+  DevPar P;
+  int rc = make_devpar(p, P, g_create_error);
+  if (rc) return rc;
+  if (p->nx < 1 || p->ny < 1 || p->nz < 1 || p->ng < 2 || !(p->cfl > 0.0)) { g_create_error = "bad grid size, ng < 2 or cfl <= 0"; return RMHD_ERR_BAD_PARAM; }
+  for (int d = 0; d < 3; ++d) if (p->bc[d] != RMHD_BC_OUTFLOW && p->bc[d] != RMHD_BC_PERIODIC) { g_create_error = "bad boundary condition"; return RMHD_ERR_BAD_PARAM; }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0 || p->device < 0 || p->device >= ndev) {
+    cudaGetLastError();
+    g_create_error = "no CUDA device (this library has no CPU fallback)";
+    return RMHD_ERR_CUDA;
+  }
+  rmhd_ctx* c = new rmhd_ctx();
+  c->p = *p; c->P = P; c->model = p->model;
+  c->nc = p->model == 0 ? R_NC : T_NC; c->nh = p->model == 0 ? R_NH : T_NH;
+  c->ns = p->model == 0 ? R_NS : T_NS; c->np = p->model == 0 ? 11 : 16;
+  c->n[0] = p->nx; c->n[1] = p->ny; c->n[2] = p->nz;
+  c->N = (size_t)p->nx * p->ny * p->nz;
+  const double lo[3] = {p->xmin, p->ymin, p->zmin}, hi[3] = {p->xmax, p->ymax, p->zmax};
+  double inv = 0.0;
+  for (int d = 0; d < 3; ++d) {
+    c->dx[d] = (hi[d] - lo[d]) / c->n[d];
+    if (c->n[d] > 1) {
+      if (!(c->dx[d] > 0.0)) { g_create_error = "empty domain"; delete c; return RMHD_ERR_BAD_PARAM; }
+      inv += 1.0 / c->dx[d];
+    }
+  }
+  c->dt = inv > 0.0 ? p->cfl / inv : p->cfl;   // G9
+  c->nsteps = 0; c->device = p->device; c->stream = (cudaStream_t)p->stream;
+  c->profiling = false;
+  for (int i = 0; i < KC_N; ++i) { c->ms[i] = 0.0; c->launches[i] = 0; }
+  c->q = c->w = c->qs = c->L1 = c->L2 = c->Ps1 = c->Ps2 = nullptr; c->d_stats = nullptr; c->h_stats = nullptr;
+  DeviceGuard dg(c->device);
+  const size_t rows = (size_t)(4 * c->nc + c->nh + 2 * c->ns);
+  cudaError_t e = cudaMalloc(&c->q, sizeof(double) * rows * c->N);
+  if (e == cudaSuccess) e = cudaMalloc(&c->d_stats, sizeof(Stats));
+  if (e == cudaSuccess) e = cudaMallocHost(&c->h_stats, sizeof(Stats));
+  if (e != cudaSuccess) { fail_cuda(nullptr, e, "allocating device state"); rmhd_destroy(c); return RMHD_ERR_CUDA; }
+  double* b = c->q;
+  b += (size_t)c->nc * c->N; c->qs = b;
+  b += (size_t)c->nc * c->N; c->L1 = b;
+  b += (size_t)c->nc * c->N; c->L2 = b;
+  b += (size_t)c->nc * c->N; c->w = b;
+  b += (size_t)c->nh * c->N; c->Ps1 = b;
+  b += (size_t)c->ns * c->N; c->Ps2 = b;
+  e = cudaMemsetAsync(c->q, 0, sizeof(double) * rows * c->N, c->stream);
+  if (e != cudaSuccess) { fail_cuda(nullptr, e, "clearing device state"); rmhd_destroy(c); return RMHD_ERR_CUDA; }
+  if (reset_stats(c)) { g_create_error = c->err; rmhd_destroy(c); return RMHD_ERR_CUDA; }
+  *out = c;
+  return RMHD_OK;
+}
+
+void rmhd_destroy(rmhd_ctx* c) {
+  if (!c) return;
+  {
+    DeviceGuard dg(c->device);
+    if (c->stream || c->q) cudaStreamSynchronize(c->stream);
+    for (auto& r : c->pending) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+    for (auto& e : c->ev_pool) cudaEventDestroy(e);
+    if (c->q) cudaFree(c->q);
+    if (c->d_stats) cudaFree(c->d_stats);
+    if (c->h_stats) cudaFreeHost(c->h_stats);
+  }
+  delete c;
+}
+
+double rmhd_dt(const rmhd_ctx* c) { return c ? c->dt : 0.0; }
+double rmhd_time(const rmhd_ctx* c) { return c ? (double)c->nsteps * c->dt : 0.0; }
+const char* rmhd_last_error(const rmhd_ctx* c) { return c ? c->err.c_str() : g_create_error.c_str(); }
+
+int rmhd_set_initial(rmhd_ctx* c, const double* prims, const double* rho_charge, int on_device) {
+  if (!c || !prims) return RMHD_ERR_BAD_PARAM;
+  DeviceGuard dg(c->device);
+  const size_t N = c->N;
+  const double* d_prims = prims;
+  const double* d_rc = rho_charge;
+  if (!on_device) {  // stage through qs (nc >= np rows) and L2 (one row)
+    CK(c, cudaMemcpyAsync(c->qs, prims, sizeof(double) * c->np * N, cudaMemcpyHostToDevice, c->stream));
+    d_prims = c->qs;
+    if (rho_charge) { CK(c, cudaMemcpyAsync(c->L2, rho_charge, sizeof(double) * N, cudaMemcpyHostToDevice, c->stream)); d_rc = c->L2; }
+  }
+  int rc = reset_stats(c);
+  if (rc) return rc;
+  const double i2[3] = {0.5 / c->dx[0], 0.5 / c->dx[1], 0.5 / c->dx[2]};
+  {
+    Timed t(c, KC_OTHER);
+    if (c->model == 0)
+      k_set_initial<0><<<blocks_for(N, 256), 256, 0, c->stream>>>(d_prims, d_rc, c->q, c->w, N, c->n[0], c->n[1], c->n[2], c->p.bc[0], c->p.bc[1], c->p.bc[2], i2[0], i2[1], i2[2], c->P, c->d_stats);
+    else
+      k_set_initial<1><<<blocks_for(N, 256), 256, 0, c->stream>>>(d_prims, nullptr, c->q, c->w, N, c->n[0], c->n[1], c->n[2], c->p.bc[0], c->p.bc[1], c->p.bc[2], i2[0], i2[1], i2[2], c->P, c->d_stats);
+    CK(c, cudaGetLastError());
+  }
+  c->nsteps = 0;
+  if ((rc = read_stats(c))) return rc;
+  if (c->h_stats->n_bad_input) { c->err = "set_initial: cells with rho <= 0, p <= 0 or |v| >= 1"; return RMHD_ERR_UNPHYSICAL_INPUT; }
+  return RMHD_OK;
+}
+
+int rmhd_set_cons(rmhd_ctx* c, const double* cons, const double* prim_guess, int on_device) {
+  if (!c || !cons) return RMHD_ERR_BAD_PARAM;
+  DeviceGuard dg(c->device);
+  const size_t N = c->N;
+  CK(c, cudaMemcpyAsync(c->q, cons, sizeof(double) * c->nc * N, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
+  const double* d_guess = prim_guess;
+  if (prim_guess && !on_device) {
+    CK(c, cudaMemcpyAsync(c->qs, prim_guess, sizeof(double) * c->nh * N, cudaMemcpyHostToDevice, c->stream));
+    d_guess = c->qs;
+  }
+  {
+    Timed t(c, KC_OTHER);
+    if (c->model == 0) k_con2prim<0><<<blocks_for(N, 256), 256, 0, c->stream>>>(c->q, d_guess, N, c->w, N, nullptr, nullptr, nullptr, N, c->P, c->d_stats);
+    else k_con2prim<1><<<blocks_for(N, 256), 256, 0, c->stream>>>(c->q, d_guess, N, c->w, N, nullptr, nullptr, nullptr, N, c->P, c->d_stats);
+    CK(c, cudaGetLastError());
+  }
+  int rc = read_stats(c);
+  if (rc) return rc;
+  return c->h_stats->n_failed ? RMHD_ERR_NONCONVERGED : RMHD_OK;
+}
+
+int rmhd_step(rmhd_ctx* c, int nsteps) {
+  if (!c || nsteps < 0) return RMHD_ERR_BAD_PARAM;
+  DeviceGuard dg(c->device);
+  if (c->model != 0) { c->err = "two-fluid stepping not built yet"; return RMHD_ERR_BAD_PARAM; }
+  for (int s = 0; s < nsteps; ++s) {
+    int rc = step_once_resistive(c);
+    if (rc) return rc;
+    c->nsteps++;
+  }
+  int rc = read_stats(c);
+  if (rc) return rc;
+  if (c->h_stats->n_failed) { c->err = "root-find failed in some cells (see rmhd_get_stats)"; return RMHD_ERR_NONCONVERGED; }
+  return RMHD_OK;
+}
+
+int rmhd_get_state(rmhd_ctx* c, double* cons, double* prims, int on_device) {
+  if (!c) return RMHD_ERR_BAD_PARAM;
+  DeviceGuard dg(c->device);
+  const size_t N = c->N;
+  const cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+  if (cons) CK(c, cudaMemcpyAsync(cons, c->q, sizeof(double) * c->nc * N, kind, c->stream));
+  if (prims) {
+    const int ib = c->model == 0 ? 5 : 10;   // B, E rows are contiguous in the conserved state
+    CK(c, cudaMemcpyAsync(prims, c->w, sizeof(double) * c->nh * N, kind, c->stream));
+    CK(c, cudaMemcpyAsync(prims + (size_t)c->nh * N, c->q + (size_t)ib * N, sizeof(double) * 6 * N, kind, c->stream));
+  }
+  CK(c, cudaStreamSynchronize(c->stream));
+  return RMHD_OK;
+}
+
+int rmhd_flux_divergence(rmhd_ctx* c, double* Lout, int on_device) {
+  if (!c || !Lout) return RMHD_ERR_BAD_PARAM;
+  DeviceGuard dg(c->device);
+  int rc = c->model == 0 ? launch_flux<0>(c, c->q, nullptr, false, c->w, c->L1) : launch_flux<1>(c, c->q, nullptr, false, c->w, c->L1);
+  if (rc) return rc;
+  CK(c, cudaMemcpyAsync(Lout, c->L1, sizeof(double) * c->nc * c->N, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
+  CK(c, cudaStreamSynchronize(c->stream));
+  resolve_events(c);
+  return RMHD_OK;
+}
+
+int rmhd_get_stats(rmhd_ctx* c, long long* hist_stage, long long* hist_c2p, int nbins, long long* n_failed, long long* first_failed_cell) {
+  if (!c || nbins < 0) return RMHD_ERR_BAD_PARAM;
+  DeviceGuard dg(c->device);
+  int rc = read_stats(c);
+  if (rc) return rc;
+  for (int b = 0; b < nbins; ++b) {
+    if (hist_stage) hist_stage[b] = 0;
+    if (hist_c2p) hist_c2p[b] = 0;
+  }
+  for (int b = 0; b < NBINS; ++b) {   // fold the library's bins into the caller's (overflow -> last bin)
+    const int t = b < nbins ? b : nbins - 1;
+    if (t < 0) break;
+    if (hist_stage) hist_stage[t] += (long long)c->h_stats->hist_stage[b];
+    if (hist_c2p) hist_c2p[t] += (long long)c->h_stats->hist_c2p[b];
+  }
+  if (n_failed) *n_failed = (long long)c->h_stats->n_failed;
+  if (first_failed_cell) *first_failed_cell = c->h_stats->first_failed == LLONG_MAX ? -1 : c->h_stats->first_failed;
+  return RMHD_OK;
+}
+
+int rmhd_set_profiling(rmhd_ctx* c, int enabled) {
+  if (!c) return RMHD_ERR_BAD_PARAM;
+  DeviceGuard dg(c->device);
+  CK(c, cudaStreamSynchronize(c->stream));
+  resolve_events(c);
+  c->profiling = enabled != 0;
+  for (int i = 0; i < KC_N; ++i) { c->ms[i] = 0.0; c->launches[i] = 0; }
+  return RMHD_OK;
+}
+
+int rmhd_get_kernel_times(rmhd_ctx* c, double* ms, long long* launches, int n) {
+  if (!c) return RMHD_ERR_BAD_PARAM;
+  DeviceGuard dg(c->device);
+  CK(c, cudaStreamSynchronize(c->stream));
+  resolve_events(c);
+  for (int i = 0; i < n; ++i) {
+    if (ms) ms[i] = i < KC_N ? c->ms[i] : 0.0;
+    if (launches) launches[i] = i < KC_N ? c->launches[i] : 0;
+  }
+  return RMHD_OK;
+}
+
+}  // extern "C"
+
+// ---- batched per-cell operations -----------------------------------------------------------
+namespace {
+struct Staging {   // device copies of host buffers for the on_device == 0 path
+  cudaStream_t s;
+  std::vector<void*> bufs;
+  explicit Staging(cudaStream_t s_) : s(s_) {}
+  ~Staging() { for (void* b : bufs) cudaFree(b); }
+  template <class T> cudaError_t in(const T* host, size_t n, const T** dev) {
+    if (!host) { *dev = nullptr; return cudaSuccess; }
+    void* d = nullptr; cudaError_t e = cudaMalloc(&d, sizeof(T) * n); if (e != cudaSuccess) return e;
+    bufs.push_back(d); *dev = (const T*)d;
+    return cudaMemcpyAsync(d, host, sizeof(T) * n, cudaMemcpyHostToDevice, s);
+  }
+  template <class T> cudaError_t out(T* host, size_t n, T** dev) {
+    if (!host) { *dev = nullptr; return cudaSuccess; }
+    void* d = nullptr; cudaError_t e = cudaMalloc(&d, sizeof(T) * n); if (e != cudaSuccess) return e;
+    bufs.push_back(d); *dev = (T*)d;
+    return cudaSuccess;
+  }
+};
+int batch_prologue(const rmhd_params* p, long long n, DevPar& P) {
+  if (!p || n < 0) { g_create_error = "bad argument"; return RMHD_ERR_BAD_PARAM; }
+  int rc = make_devpar(p, P, g_create_error);
+  if (rc) return rc;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0 || p->device < 0 || p->device >= ndev) {
+    cudaGetLastError(); g_create_error = "no CUDA device (this library has no CPU fallback)"; return RMHD_ERR_CUDA;
+  }
+  return RMHD_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int rmhd_stage_batch(const rmhd_params* p, long long ncells, const double* q_ex, const double* prim_guess,
+                     const double* sigma_cell, double a_dt, double* q_out, double* prims_out, int* iters, int* fail,
+                     int on_device) {
+  DevPar P;
+  int rc = batch_prologue(p, ncells, P);
+  if (rc) return rc;
+  if (!q_ex || !prim_guess || !q_out || !prims_out) { g_create_error = "null buffer"; return RMHD_ERR_BAD_PARAM; }
+  if (p->model != RMHD_RESISTIVE) { g_create_error = "two-fluid stage batch not built yet"; return RMHD_ERR_BAD_PARAM; }
+  if (ncells == 0) return RMHD_OK;
+  DeviceGuard dg(p->device);
+  cudaStream_t s = (cudaStream_t)p->stream;
+  const size_t N = (size_t)ncells;
+  const int nc = 14, np = 11;
+  Staging st(s);
+  const double *d_qex = q_ex, *d_pg = prim_guess, *d_sig = sigma_cell;
+  double *d_qo = q_out, *d_po = prims_out; int *d_it = iters, *d_fl = fail;
+  if (!on_device) {
+    CK(nullptr, st.in(q_ex, nc * N, &d_qex)); CK(nullptr, st.in(prim_guess, np * N, &d_pg)); CK(nullptr, st.in(sigma_cell, N, &d_sig));
+    CK(nullptr, st.out(q_out, nc * N, &d_qo)); CK(nullptr, st.out(prims_out, np * N, &d_po));
+    CK(nullptr, st.out(iters, N, &d_it)); CK(nullptr, st.out(fail, N, &d_fl));
+  }
+  k_stage_batch_resistive<<<blocks_for(N, 128), 128, 0, s>>>(d_qex, d_pg, d_sig, a_dt, d_qo, d_po, d_it, d_fl, N, P);
+  CK(nullptr, cudaGetLastError());
+  if (!on_device) {
+    CK(nullptr, cudaMemcpyAsync(q_out, d_qo, sizeof(double) * nc * N, cudaMemcpyDeviceToHost, s));
+    CK(nullptr, cudaMemcpyAsync(prims_out, d_po, sizeof(double) * np * N, cudaMemcpyDeviceToHost, s));
+    if (iters) CK(nullptr, cudaMemcpyAsync(iters, d_it, sizeof(int) * N, cudaMemcpyDeviceToHost, s));
+    if (fail) CK(nullptr, cudaMemcpyAsync(fail, d_fl, sizeof(int) * N, cudaMemcpyDeviceToHost, s));
+    CK(nullptr, cudaStreamSynchronize(s));
+  }
+  return RMHD_OK;
+}
+
+int rmhd_prim2cons_batch(const rmhd_params* p, long long ncells, const double* prims, const double* rho_charge, double* cons,
+                         int on_device) {
+  DevPar P;
+  int rc = batch_prologue(p, ncells, P);
+  if (rc) return rc;
+  if (!prims || !cons) { g_create_error = "null buffer"; return RMHD_ERR_BAD_PARAM; }
+  if (ncells == 0) return RMHD_OK;
+  DeviceGuard dg(p->device);
+  cudaStream_t s = (cudaStream_t)p->stream;
+  const size_t N = (size_t)ncells;
+  const int nc = p->model == 0 ? 14 : 18, np = p->model == 0 ? 11 : 16;
+  Staging st(s);
+  const double *d_pr = prims, *d_rc = rho_charge; double* d_co = cons;
+  if (!on_device) { CK(nullptr, st.in(prims, np * N, &d_pr)); CK(nullptr, st.in(rho_charge, N, &d_rc)); CK(nullptr, st.out(cons, nc * N, &d_co)); }
+  if (p->model == 0) k_prim2cons_batch<0><<<blocks_for(N, 256), 256, 0, s>>>(d_pr, d_rc, d_co, N, P);
+  else k_prim2cons_batch<1><<<blocks_for(N, 256), 256, 0, s>>>(d_pr, nullptr, d_co, N, P);
+  CK(nullptr, cudaGetLastError());
+  if (!on_device) { CK(nullptr, cudaMemcpyAsync(cons, d_co, sizeof(double) * nc * N, cudaMemcpyDeviceToHost, s)); CK(nullptr, cudaStreamSynchronize(s)); }
+  return RMHD_OK;
+}
+
+int rmhd_con2prim_batch(const rmhd_params* p, long long ncells, const double* cons, const double* prim_guess, double* prims,
+                        int* iters, int* fail, int on_device) {
+  DevPar P;
+  int rc = batch_prologue(p, ncells, P);
+  if (rc) return rc;
+  if (!cons || !prims) { g_create_error = "null buffer"; return RMHD_ERR_BAD_PARAM; }
+  if (ncells == 0) return RMHD_OK;
+  DeviceGuard dg(p->device);
+  cudaStream_t s = (cudaStream_t)p->stream;
+  const size_t N = (size_t)ncells;
+  const int nc = p->model == 0 ? 14 : 18, np = p->model == 0 ? 11 : 16, nh = p->model == 0 ? 5 : 10;
+  Staging st(s);
+  const double *d_co = cons, *d_pg = prim_guess; double* d_pr = prims; int *d_it = iters, *d_fl = fail;
+  if (!on_device) {
+    CK(nullptr, st.in(cons, nc * N, &d_co)); CK(nullptr, st.in(prim_guess, np * N, &d_pg)); CK(nullptr, st.out(prims, np * N, &d_pr));
+    CK(nullptr, st.out(iters, N, &d_it)); CK(nullptr, st.out(fail, N, &d_fl));
+  }
+  if (p->model == 0) k_con2prim<0><<<blocks_for(N, 256), 256, 0, s>>>(d_co, d_pg, N, d_pr, N, d_pr + (size_t)nh * N, d_it, d_fl, N, P, nullptr);
+  else k_con2prim<1><<<blocks_for(N, 256), 256, 0, s>>>(d_co, d_pg, N, d_pr, N, d_pr + (size_t)nh * N, d_it, d_fl, N, P, nullptr);
+  CK(nullptr, cudaGetLastError());
+  if (!on_device) {
+    CK(nullptr, cudaMemcpyAsync(prims, d_pr, sizeof(double) * np * N, cudaMemcpyDeviceToHost, s));
+    if (iters) CK(nullptr, cudaMemcpyAsync(iters, d_it, sizeof(int) * N, cudaMemcpyDeviceToHost, s));
+    if (fail) CK(nullptr, cudaMemcpyAsync(fail, d_fl, sizeof(int) * N, cudaMemcpyDeviceToHost, s));
+    CK(nullptr, cudaStreamSynchronize(s));
+  }
+  return RMHD_OK;
+}
+
+// ---- probes ----------------------------------------------------------------------------------
+int rmhd_probe_fp64(int device, void* stream, double* tflops) {
+  if (!tflops) return RMHD_ERR_BAD_PARAM;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { cudaGetLastError(); g_create_error = "no CUDA device"; return RMHD_ERR_CUDA; }
+  DeviceGuard dg(device);
+  cudaStream_t s = (cudaStream_t)stream;
+  cudaDeviceProp prop; CK(nullptr, cudaGetDeviceProperties(&prop, device));
+  const int blocks = prop.multiProcessorCount * 8, threads = 256, iters = 1 << 15;
+  double* d = nullptr; CK(nullptr, cudaMalloc(&d, sizeof(double) * blocks * threads));
+  cudaEvent_t a, b; cudaEventCreate(&a); cudaEventCreate(&b);
+  double best = 0.0;
+  for (int rep = 0; rep < 5; ++rep) {
+    cudaEventRecord(a, s);
+    k_probe_fp64<<<blocks, threads, 0, s>>>(d, iters, 1.0 + rep);
+    cudaEventRecord(b, s);
+    cudaError_t e = cudaEventSynchronize(b);
+    if (e != cudaSuccess) { cudaFree(d); return fail_cuda(nullptr, e, "fp64 probe"); }
+    float ms; cudaEventElapsedTime(&ms, a, b);
+    const double fl = 2.0 * 8.0 * (double)iters * blocks * threads;
+    if (rep > 0) best = fmax(best, fl / (ms * 1e-3) * 1e-12);
+  }
+  cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(d);
+  *tflops = best;
+  return RMHD_OK;
+}
+
+int rmhd_probe_hbm(int device, void* stream, long long bytes, double* gbs) {
+  if (!gbs || bytes < 1024) return RMHD_ERR_BAD_PARAM;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { cudaGetLastError(); g_create_error = "no CUDA device"; return RMHD_ERR_CUDA; }
+  DeviceGuard dg(device);
+  cudaStream_t s = (cudaStream_t)stream;
+  cudaDeviceProp prop; CK(nullptr, cudaGetDeviceProperties(&prop, device));
+  const size_t n2 = (size_t)bytes / sizeof(double2);
+  double2 *src = nullptr, *dst = nullptr;
+  CK(nullptr, cudaMalloc(&src, n2 * sizeof(double2)));
+  cudaError_t e = cudaMalloc(&dst, n2 * sizeof(double2));
+  if (e != cudaSuccess) { cudaFree(src); return fail_cuda(nullptr, e, "hbm probe alloc"); }
+  cudaMemsetAsync(src, 1, n2 * sizeof(double2), s);
+  cudaEvent_t a, b; cudaEventCreate(&a); cudaEventCreate(&b);
+  double best = 0.0;
+  for (int rep = 0; rep < 6; ++rep) {
+    cudaEventRecord(a, s);
+    k_probe_copy<<<prop.multiProcessorCount * 16, 256, 0, s>>>(src, dst, n2);
+    cudaEventRecord(b, s);
+    e = cudaEventSynchronize(b);
+    if (e != cudaSuccess) break;
+    float ms; cudaEventElapsedTime(&ms, a, b);
+    if (rep > 0) best = fmax(best, 2.0 * n2 * sizeof(double2) / (ms * 1e-3) * 1e-9);
+  }
+  cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(src); cudaFree(dst);
+  if (e != cudaSuccess) return fail_cuda(nullptr, e, "hbm probe");
+  *gbs = best;
+  return RMHD_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,282 @@
+"""Parity of the CUDA path (through the C-ABI) against the CPU oracle, element by element on
+the same seeded inputs.  Run on the B200 box:  python -m pytest tests -m gpu
+
+Tolerances: per-cell algebra 1e-12..1e-13 relative; config
+runs use BASELINE.json's rel-L1 bounds (cfg1 1e-9, cfg2 1e-10, cfg3/4/5 1e-8), where
+rel-L1 = sum |q_gpu - q_oracle| / sum |q_oracle| over all conserved variables and cells.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+G43 = 4.0 / 3.0
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("-m gpu tests need a CUDA device (there is no CPU fallback)")
+    from paper_1808_09721_b200 import build, binding
+    build.build()
+    binding.lib()
+    return binding
+
+
+def rel_l1(a, b):
+    return np.abs(a - b).sum() / np.abs(b).sum()
+
+
+def run_gpu(B, cfg, nsteps=None, params_override=None):
+    kw = dict(cfg["params"])
+    if params_override:
+        kw.update(params_override)
+    sim = B.Rmhd(**kw)
+    sim.set_initial(np.ascontiguousarray(cfg["prims"]), cfg.get("rho_charge"))
+    sim.step(cfg["nsteps"] if nsteps is None else nsteps)
+    cons, prims = sim.get_state()
+    stats = sim.stats()
+    sim.close()
+    return cons, prims, stats
+
+
+def run_oracle(O, cfg, nsteps=None, params_override=None):
+    kw = dict(cfg["params"])
+    if params_override:
+        kw.update(params_override)
+    S = O.OracleSim(O.make_params(**kw))
+    S.set_initial(cfg["prims"], cfg.get("rho_charge"))
+    rc = S.step(cfg["nsteps"] if nsteps is None else nsteps)
+    cons, prims = S.get_state()
+    stats = S.get_stats()
+    S.close()
+    assert rc == 0
+    return cons, prims, stats
+
+
+# ------------------------------------------------------------------------------------------
+# per-cell kernels
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n", [0, 1, 33, 4099])
+def test_prim2cons_con2prim_batch_resistive(B, O, synth, n):
+    w = synth.random_resistive_prims(n, seed=3, vmax=0.99)
+    rc = np.random.default_rng(1).standard_normal(n)
+    P = B.make_params(model=0, gamma=G43)
+    PO = O.make_params(model=0, gamma=G43)
+    q = np.empty((14, n))
+    B.rmhd_prim2cons_batch(P, w, q, rc)
+    if n == 0:
+        return
+    qo = O.prim2cons(PO, w, rc)
+    assert rel_l1(q, qo) < 1e-14
+    assert (np.abs(q - qo) / np.abs(qo[:5]).max(axis=0)).max() < 1e-14
+    # con2prim on the oracle's conserved state, no guess
+    w2 = np.empty((11, n)); it = np.zeros(n, np.int32); fl = np.zeros(n, np.int32)
+    B.rmhd_con2prim_batch(P, qo, w2, None, it, fl)
+    wo, ito, flo = O.con2prim(PO, qo)
+    assert not fl.any() and not flo.any()
+    W2 = 1.0 / (1.0 - (w[1:4] ** 2).sum(0))
+    cond = W2 * (1.0 + w[0] * (1 + 4 * w[4] / w[0]) / w[4])
+    assert (np.abs(w2[:5] - wo[:5]) / np.maximum(np.abs(wo[:5]), 1e-3) / cond).max() < 1e-13
+    assert np.array_equal(w2[5:], wo[5:])
+    assert np.abs(it - ito).max() <= 1
+
+
+def test_prim2cons_con2prim_batch_two_fluid(B, O, synth):
+    n = 5000
+    w = synth.random_two_fluid_prims(n, seed=5, vmax=0.9)
+    kw = dict(model=1, gamma=G43, mu_e=-100.0, mu_p=100.0)
+    P, PO = B.make_params(**kw), O.make_params(**kw)
+    q = np.empty((18, n))
+    B.rmhd_prim2cons_batch(P, w, q)
+    qo = O.prim2cons(PO, w)
+    assert (np.abs(q - qo) / np.abs(qo[:10]).max(axis=0)).max() < 1e-14
+    w2 = np.empty((16, n)); it = np.zeros(n, np.int32); fl = np.zeros(n, np.int32)
+    B.rmhd_con2prim_batch(P, qo, w2, w, it, fl)
+    wo, ito, flo = O.con2prim(PO, qo, w)
+    assert not fl.any() and not flo.any()
+    assert (np.abs(w2 - wo) / np.maximum(np.abs(wo), 1e-2)).max() < 1e-9      # both sit at the same root
+    assert rel_l1(w2, wo) < 1e-13
+
+
+# ------------------------------------------------------------------------------------------
+# config 2: batched implicit stage
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n", [1, 31, 2 ** 16 + 37])
+def test_config2_stage_batch_parity(B, O, synth, n):
+    c = synth.config2(n, seed=0)
+    P = B.make_params(**c["params"]); PO = O.make_params(**c["params"])
+    w = c["prims"]; sig = c["sigma_cell"]; a = c["a_dt"]
+    q_ex = O.prim2cons(PO, w)       # identical input to both sides
+    qo, wo, ito, flo = O.stage_batch(PO, q_ex, w, a, sig)
+    q = np.empty_like(q_ex); wg = np.empty_like(w); it = np.zeros(n, np.int32); fl = np.zeros(n, np.int32)
+    B.rmhd_stage_batch(P, q_ex, w, a, q, wg, sig, it, fl)
+    ok = (fl == 0) & (flo == 0)
+    assert (fl != 0).sum() <= max(1, 1e-5 * n) and (flo != 0).sum() <= max(1, 1e-5 * n)
+    assert ((fl != 0) != (flo != 0)).sum() <= max(1, 1e-5 * n)
+    assert rel_l1(q[:, ok], qo[:, ok]) <= 1e-10          # BASELINE.json configs[1] tolerance
+    assert rel_l1(q[:, ok], qo[:, ok]) <= 1e-14          # in fact both sit at round-off
+    assert np.abs(q[8:11, ok] - qo[8:11, ok]).max() < 1e-12
+    assert rel_l1(wg[:, ok], wo[:, ok]) < 1e-13
+    assert it[ok].min() >= 1 and it[ok].max() <= 12
+
+
+def test_config2_device_buffers_and_own_prim2cons(B, O, synth):
+    """Same call with torch CUDA tensors (the launch configuration bench.py times), q_ex made by the
+    library's own prim2cons."""
+    import torch
+    n = 2 ** 16
+    c = synth.config2(n, seed=0)
+    P = B.make_params(**c["params"]); PO = O.make_params(**c["params"])
+    dev = torch.device("cuda", 0)
+    w = torch.from_numpy(c["prims"]).to(dev); sig = torch.from_numpy(c["sigma_cell"]).to(dev)
+    q_ex = torch.empty((14, n), dtype=torch.float64, device=dev)
+    B.rmhd_prim2cons_batch(P, w, q_ex)
+    q = torch.empty_like(q_ex); wg = torch.empty_like(w)
+    it = torch.zeros(n, dtype=torch.int32, device=dev); fl = torch.zeros(n, dtype=torch.int32, device=dev)
+    B.rmhd_stage_batch(P, q_ex, w, c["a_dt"], q, wg, sig, it, fl)
+    torch.cuda.synchronize()
+    qo, wo, ito, flo = O.stage_batch(PO, O.prim2cons(PO, c["prims"]), c["prims"], c["a_dt"], c["sigma_cell"])
+    ok = (fl.cpu().numpy() == 0) & (flo == 0)
+    assert ok.mean() > 1 - 1e-5
+    assert rel_l1(q.cpu().numpy()[:, ok], qo[:, ok]) <= 1e-10
+
+
+# ------------------------------------------------------------------------------------------
+# L(q): flux-vector splitting + WENO3 + divergence, virtual ghost zones
+# ------------------------------------------------------------------------------------------
+def _random_state(model, shape, seed):
+    rng = np.random.default_rng(seed)
+    nz, ny, nx = shape
+    np_ = 11 if model == 0 else 16
+    w = np.zeros((np_, nz, ny, nx))
+    for s in range(1 if model == 0 else 2):
+        w[5 * s] = 10 ** rng.uniform(-0.5, 0.5, shape)
+        w[5 * s + 4] = 10 ** rng.uniform(-1, 0.5, shape)
+        w[5 * s + 1:5 * s + 4] = rng.uniform(-0.5, 0.5, (3,) + shape)
+    w[-6:] = 0.3 * rng.standard_normal((6,) + shape)
+    return w
+
+
+@pytest.mark.parametrize("model,shape,bc", [
+    (0, (1, 1, 67), (0, 0, 0)), (0, (1, 1, 130), (1, 1, 1)), (0, (1, 9, 70), (1, 0, 0)), (0, (1, 33, 5), (0, 1, 0)),
+    (0, (7, 10, 35), (0, 1, 0)), (0, (11, 3, 66), (1, 0, 1)), (0, (9, 1, 40), (0, 0, 1)),
+    (1, (1, 1, 67), (1, 0, 0)), (1, (1, 12, 37), (0, 1, 0)), (1, (6, 9, 34), (1, 1, 0)),
+])
+def test_flux_divergence_parity(B, O, model, shape, bc):
+    nz, ny, nx = shape
+    w = _random_state(model, shape, seed=nx + 7 * ny + 13 * nz)
+    kw = dict(model=model, nx=nx, ny=ny, nz=nz, bc=bc, xlim=(0.0, 1.0), ylim=(-1.0, 0.5), zlim=(0.0, 0.7), gamma=G43,
+              sigma=25.0, eta=1e-3, mu_e=-20.0, mu_p=10.0)
+    rc = np.random.default_rng(0).standard_normal(shape) if model == 0 else None
+    sim = B.Rmhd(**kw); sim.set_initial(w, rc)
+    L = sim.flux_divergence()
+    q, _ = sim.get_state()
+    sim.close()
+    S = O.OracleSim(O.make_params(**kw)); S.set_initial(w, rc)
+    Lo = S.eval_L(); qo, _ = S.get_state()
+    assert (np.abs(q - qo) / (np.abs(qo).max() + 1)).max() < 1e-14
+    scale = np.abs(Lo).max(axis=(1, 2, 3), keepdims=True) + 1e-30
+    assert (np.abs(L - Lo) / scale).max() < 1e-12, np.unravel_index(np.argmax(np.abs(L - Lo) / scale), L.shape)
+
+
+def test_gauss_law_initialisation_matches(B, O, synth):
+    c = synth.config3(nx=48, ny=40, nsteps=1)
+    q, _, _ = run_gpu(B, c, nsteps=0)
+    qo, _, _ = run_oracle(O, c, nsteps=0)
+    assert np.abs(qo[11]).max() > 1.0          # the shear layer carries charge (G10)
+    assert np.abs(q[11] - qo[11]).max() < 1e-12 * np.abs(qo[11]).max()
+
+
+# ------------------------------------------------------------------------------------------
+# full configs
+# ------------------------------------------------------------------------------------------
+def test_config1_riemann_tube_full(B, O, synth):
+    c = synth.config1()
+    q, w, st = run_gpu(B, c)
+    qo, wo, sto = run_oracle(O, c)
+    assert st["n_failed"] == 0
+    assert rel_l1(q, qo) <= 1e-9, rel_l1(q, qo)
+    assert st["hist_stage"].sum() == 2 * 128 * 128 and st["hist_c2p"].sum() == 128 * 128
+    assert st["hist_stage"][0] == 0
+
+
+def test_config3_shear_layer_reduced(B, O, synth):
+    c = synth.config3(nx=96, ny=128, nsteps=60)
+    q, w, st = run_gpu(B, c)
+    qo, wo, _ = run_oracle(O, c)
+    assert st["n_failed"] == 0
+    assert rel_l1(q, qo) <= 1e-8, rel_l1(q, qo)
+    assert rel_l1(w[:5], wo[:5]) <= 1e-8
+
+
+def test_config5_blast_reduced(B, O, synth):
+    c = synth.config5(n=40, nsteps=20)
+    q, w, st = run_gpu(B, c)
+    qo, wo, _ = run_oracle(O, c)
+    assert st["n_failed"] == 0
+    assert rel_l1(q, qo) <= 1e-8, rel_l1(q, qo)
+
+
+def test_config5_full_size_sampled_against_oracle(B, O, synth):
+    """256^3, the launch configuration bench.py times.  Two steps; the oracle recomputes a
+    sub-box (24^3 + 8 halo cells per side, enough for 2 steps x 2 stages x 2-cell stencil) that
+    straddles the blast edge, from the same initial data; plus properties that hold at any size."""
+    n = 256
+    c = synth.config5(n=n, nsteps=2)
+    sim = B.Rmhd(**c["params"])
+    sim.set_initial(c["prims"])
+    q0, _ = sim.get_state()
+    sim.step(2)
+    q, w = sim.get_state()
+    st = sim.stats()
+    sim.close()
+    assert st["n_failed"] == 0
+    lo, m, h = 136, 24, 8            # box [136,160)^3 ; blast edge at 128 + 25.6 cells
+    sl = slice(lo - h, lo + m + h)
+    sub = dict(c); P = dict(c["params"]); dx = 1.0 / n
+    P.update(nx=m + 2 * h, ny=m + 2 * h, nz=m + 2 * h,
+             xlim=(-0.5 + (lo - h) * dx, -0.5 + (lo + m + h) * dx),
+             ylim=(-0.5 + (lo - h) * dx, -0.5 + (lo + m + h) * dx),
+             zlim=(-0.5 + (lo - h) * dx, -0.5 + (lo + m + h) * dx))
+    sub["params"] = P
+    sub["prims"] = np.ascontiguousarray(c["prims"][:, sl, sl, sl])
+    qo, wo, _ = run_oracle(O, sub, nsteps=2)
+    inner = slice(h, h + m)
+    a = q[:, lo:lo + m, lo:lo + m, lo:lo + m]; b = qo[:, inner, inner, inner]
+    assert np.abs(b[1]).max() > 1e-4                     # the box does see the blast wave
+    assert rel_l1(a, b) <= 1e-8, rel_l1(a, b)
+    # properties at full size: source-free rows conserved (nothing reaches the boundary) ...
+    for r in (0, 4, 5):
+        assert abs(q[r].sum() - q0[r].sum()) <= 1e-12 * np.abs(q0[r]).sum()
+    # ... and x-mirror symmetry (B_x even): S_x odd, D even
+    assert np.abs(q[0] - q[0][:, :, ::-1]).max() < 1e-11
+    assert np.abs(q[1] + q[1][:, :, ::-1]).max() < 1e-11
+
+
+# ------------------------------------------------------------------------------------------
+# API behaviour
+# ------------------------------------------------------------------------------------------
+def test_unphysical_input_is_reported(B, synth):
+    c = synth.config1(nx=16)
+    w = c["prims"].copy(); w[4, 0, 0, 3] = -1.0
+    sim = B.Rmhd(**c["params"])
+    with pytest.raises(B.RmhdError) as e:
+        sim.set_initial(w)
+    assert e.value.code == B.RMHD_ERR_UNPHYSICAL_INPUT
+    sim.close()
+
+
+def test_set_cons_get_state_round_trip_and_device_buffers(B, O, synth):
+    import torch
+    c = synth.config3(nx=32, ny=24, nsteps=3)
+    sim = B.Rmhd(**c["params"]); sim.set_initial(c["prims"]); sim.step(3)
+    q, w = sim.get_state()
+    qd, wd = sim.get_state(device=True)
+    assert np.array_equal(qd.cpu().numpy(), q) and np.array_equal(wd.cpu().numpy(), w)
+    # restart from the checkpoint on a new context: same continuation
+    sim.step(2); q5, _ = sim.get_state(); sim.close()
+    sim2 = B.Rmhd(**c["params"]); assert sim2.set_cons(q, w) == 0; sim2.step(2); q5b, _ = sim2.get_state(); sim2.close()
+    assert rel_l1(q5b, q5) < 1e-13
+    assert abs(B.Rmhd(**c["params"]).dt - 0.4 / (32 / 1.0 + 24 / 2.0)) < 1e-16

@@ -377,3 +377,40 @@ def test_two_fluid_stage_residual_and_fixed_rows(O, synth):
     assert (np.abs(R).max(0) / scale).max() < 1e-12
     # psi*, phi* closed forms with rhoc = Dbar
     assert np.allclose(q[16], (q_ex[16] + a * q_ex[5]) / (1 + a), rtol=1e-12, atol=1e-14)
+
+
+def test_two_fluid_flux_is_sum_of_single_fluid_hydro_fluxes(O, synth):
+    """(A1) P:L443 with G2: without fields the two-fluid flux rows are the plain / mu-weighted
+    sums of the two species' single-fluid hydro fluxes (computed by the resistive model, itself
+    pinned against textbook values above); with the fluid at rest they are the Maxwell rows."""
+    n = 300
+    w = synth.random_two_fluid_prims(n, seed=21, vmax=0.8)
+    w[10:16] = 0.0
+    mu_e, mu_p = -7.0, 3.0
+    P2 = O.make_params(model=1, gamma=G43, mu_e=mu_e, mu_p=mu_p)
+    P1 = O.make_params(model=0, gamma=G43, sigma=0.0)
+    q2 = O.prim2cons(P2, w)
+    zeros = np.zeros((6, n))
+    fs = []
+    for s in range(2):
+        w1 = np.concatenate([w[5 * s:5 * s + 5], zeros])
+        q1 = O.prim2cons(P1, w1)
+        fs.append([O.flux_vector(P1, k, q1, w1) for k in range(3)])
+    for k in range(3):
+        f = O.flux_vector(P2, k, q2, w)
+        fe, fp = fs[0][k], fs[1][k]
+        assert np.allclose(f[0:5], fe[0:5] + fp[0:5], rtol=1e-12, atol=1e-13)
+        assert np.allclose(f[5:10], mu_e * fe[0:5] + mu_p * fp[0:5], rtol=1e-12, atol=1e-12)
+        assert np.all(f[10:] == 0.0)
+    # fields only, species at rest: Maxwell rows identical to the resistive model's
+    rng = np.random.default_rng(2)
+    E = rng.standard_normal((3, n)); B = rng.standard_normal((3, n))
+    w[1:4] = 0.0; w[6:9] = 0.0; w[10:13] = B; w[13:16] = E
+    q2 = O.prim2cons(P2, w); q2[16] = rng.standard_normal(n); q2[17] = rng.standard_normal(n)
+    w1 = np.concatenate([w[0:1] + w[5:6], np.zeros((3, n)), w[4:5] + w[9:10], B, E])
+    q1 = O.prim2cons(P1, w1); q1[12] = q2[16]; q1[13] = q2[17]
+    for k in range(3):
+        f = O.flux_vector(P2, k, q2, w); f1 = O.flux_vector(P1, k, q1, w1)
+        assert np.allclose(f[1:5], f1[1:5], rtol=1e-12, atol=1e-13)      # stress + Poynting
+        assert np.array_equal(f[10:16], f1[5:11])                          # Faraday / Ampere rows
+        assert np.array_equal(f[16], f1[12]) and np.array_equal(f[17], f1[13])
