@@ -31,6 +31,7 @@ def build(force=False, verbose=False):
            "-shared", "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include"), "-o", LIB] + SOURCES
     if verbose:
         cmd += ["-Xptxas", "-v"]
+    cmd += os.environ.get("RMHD_NVCC_FLAGS", "").split()
     subprocess.check_call(cmd)
     return LIB
 

@@ -354,6 +354,103 @@ __global__ void __launch_bounds__(FLUX_THREADS, 2) k_flux(ConsRows<MODEL> qin, H
 }
 
 // =======================================================================================
+// a4, axes 1 and 2 (sweep axis strided in memory): MARCHING kernel.  Lanes run along x, so the
+// stencil never crosses lanes: each thread owns one (x, other) column and marches along the
+// sweep axis over a segment, keeping the 3-cell f+ / 2-cell f- window of its column in shared
+// memory (used as per-thread scratch: no barrier anywhere in the kernel) and the previous
+// face flux in registers.  Per new cell c: load q, w (boundary index map), flux vector,
+// f+- = (f +- q)/2, face between c-2 and c-1 by WENO3, then L of cell c-2.  The next cell's
+// inputs are loaded before the current cell's arithmetic (software prefetch).
+// =======================================================================================
+#ifndef RMHD_MARCH_MINB
+#define RMHD_MARCH_MINB 3
+#endif
+constexpr int MARCH_THREADS = 128;
+template <int MODEL> constexpr size_t march_smem_bytes() { return sizeof(double) * 5 * Dim<MODEL>::NC * MARCH_THREADS; }
+
+template <int MODEL, int AXIS>
+__global__ void __launch_bounds__(MARCH_THREADS, MODEL == 0 ? RMHD_MARCH_MINB : 2)
+k_flux_march(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, size_t N, int nx, int ny, int nz, int bc,
+             double inv_dx, int accumulate, int seg_len, DevPar P) {
+  static_assert(AXIS == 1 || AXIS == 2, "marching kernel is for the strided axes");
+  constexpr int NC = Dim<MODEL>::NC, NH = Dim<MODEL>::NH, T = MARCH_THREADS;
+  extern __shared__ double sm[];   // f+ ring [3][NC][T], f- ring [2][NC][T]
+  const int i = blockIdx.x * T + threadIdx.x;
+  if (i >= nx) return;
+  const int other = blockIdx.y;
+  const int ns = AXIS == 1 ? ny : nz;
+  const int s_begin = blockIdx.z * seg_len;
+  const int s_end = min(ns, s_begin + seg_len);
+  const size_t stride = AXIS == 1 ? (size_t)nx : (size_t)nx * ny;
+  const size_t base = AXIS == 1 ? (size_t)other * ny * nx + i : (size_t)other * nx + i;
+  double* ring = sm + threadIdx.x;
+  int a0 = 0, a1 = NC * T, a2 = 2 * NC * T;            // f+ slots of cells c-3, c-2, c-1
+  int b0 = 3 * NC * T, b1 = 4 * NC * T;                // f- slots of cells c-2, c-1
+
+  double qc[NC], wc[NH], qn_[NC], wn_[NH];
+  auto load = [&](int c, double* q_, double* w_) {
+    const size_t idx = base + (size_t)bc_map(c, ns, bc) * stride;
+#pragma unroll
+    for (int v = 0; v < NC; ++v) q_[v] = __ldg(qin.r[v] + idx);
+#pragma unroll
+    for (int v = 0; v < NH; ++v) w_[v] = __ldg(win.r[v] + idx);
+  };
+  // prologue: cells s_begin-2, s_begin-1, s_begin
+  load(s_begin - 2, qn_, wn_);
+#pragma unroll 1
+  for (int c = s_begin - 2; c <= s_begin; ++c) {
+#pragma unroll
+    for (int v = 0; v < NC; ++v) qc[v] = qn_[v];
+#pragma unroll
+    for (int v = 0; v < NH; ++v) wc[v] = wn_[v];
+    load(c + 1, qn_, wn_);
+    double f[NC];
+    if (MODEL == 0) r_flux<AXIS>(qc, wc, P.sigma, P, f); else t_flux<AXIS>(qc, wc, P, f);
+#pragma unroll
+    for (int v = 0; v < NC; ++v) {
+      ring[a0 + v * T] = 0.5 * (f[v] + qc[v]);
+      ring[b0 + v * T] = 0.5 * (f[v] - qc[v]);   // for c = s_begin-2 this slot is overwritten next
+    }
+    { const int t = a0; a0 = a1; a1 = a2; a2 = t; }
+    { const int t = b0; b0 = b1; b1 = t; }
+  }
+  double Fp[NC], La[NC];
+  // main loop: new cell c, face between c-2 and c-1, L of cell c-2
+#pragma unroll 1
+  for (int c = s_begin + 1; c <= s_end + 1; ++c) {
+#pragma unroll
+    for (int v = 0; v < NC; ++v) qc[v] = qn_[v];
+#pragma unroll
+    for (int v = 0; v < NH; ++v) wc[v] = wn_[v];
+    const bool emit = c >= s_begin + 2;
+    const size_t oidx = base + (size_t)(emit ? c - 2 : 0) * stride;
+    // issue every global load of this step up front: next cell's inputs and the partial L to add to
+    if (c <= s_end) load(c + 1, qn_, wn_);
+    if (accumulate && emit) {
+#pragma unroll
+      for (int v = 0; v < NC; ++v) La[v] = L[(size_t)v * N + oidx];
+    } else {
+#pragma unroll
+      for (int v = 0; v < NC; ++v) La[v] = 0.0;
+    }
+    double f[NC];
+    if (MODEL == 0) r_flux<AXIS>(qc, wc, P.sigma, P, f); else t_flux<AXIS>(qc, wc, P, f);
+#pragma unroll
+    for (int v = 0; v < NC; ++v) {
+      const double fpc = 0.5 * (f[v] + qc[v]);
+      const double fmc = 0.5 * (f[v] - qc[v]);
+      const double F = weno3(ring[a0 + v * T], ring[a1 + v * T], ring[a2 + v * T]) + weno3(fmc, ring[b1 + v * T], ring[b0 + v * T]);
+      if (emit) L[(size_t)v * N + oidx] = La[v] - (F - Fp[v]) * inv_dx;
+      Fp[v] = F;
+      ring[a0 + v * T] = fpc;
+      ring[b0 + v * T] = fmc;
+    }
+    { const int t = a0; a0 = a1; a1 = a2; a2 = t; }
+    { const int t = b0; b0 = b1; b1 = t; }
+  }
+}
+
+// =======================================================================================
 // C + P: q^{n+1} = qn + dt/2 (L1 + L2) + dt/2 (Psi1 + Psi2)  (eq 11), then con2prim.
 // SRC_ROWS: for MODEL 0 rows 8,9,10,12,13 ; MODEL 1 rows 6..9, 13..17
 // =======================================================================================

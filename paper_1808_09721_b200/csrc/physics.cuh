@@ -273,15 +273,33 @@ RMHD_DEV void t_source7(const double* De /*D_e, D_p*/, const Hyd* h, const doubl
 }
 
 // ---------------------------------------------------------------------------------------
-// WENO3 (Shu 1997, r = 2; G7), one division: value at the face between b and c biased to a.
-//   alpha0 = (2/3)/(eps+beta0)^2, alpha1 = (1/3)/(eps+beta1)^2 scaled by 3 (eps+beta0)^2 (eps+beta1)^2
+// WENO3 (Shu 1997, r = 2; G7): value at the face between b and c biased to a.
+//   beta0 = (c-b)^2, beta1 = (b-a)^2, alpha0 = (2/3)/(eps+beta0)^2, alpha1 = (1/3)/(eps+beta1)^2
+//   u = (alpha0 (b+c)/2 + alpha1 (3b-a)/2)/(alpha0+alpha1) = b + ( d1 + w0 (d0 - d1) )/2,
+//   w0 = alpha0/(alpha0+alpha1) = 2 e1^2 / (2 e1^2 + e0^2),  e_k = eps + beta_k
+// One reciprocal per reconstruction: MUFU seed (rcp.approx.ftz.f64, ~2^-23) + 3 Newton steps
+// (full double accuracy; the denominator is >= eps^2 = 1e-12, never denormal).
 // ---------------------------------------------------------------------------------------
+RMHD_DEV double fast_rcp(double x) {
+#ifdef __CUDA_ARCH__
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  double e = fma(-x, r, 1.0); r = fma(r, e, r);
+  e = fma(-x, r, 1.0); r = fma(r, e, r);
+  e = fma(-x, r, 1.0); r = fma(r, e, r);
+  return r;
+#else
+  return 1.0 / x;
+#endif
+}
+
 RMHD_DEV double weno3(double a, double b, double c) {
   const double eps = 1e-6;
   const double d0 = c - b, d1 = b - a;
-  const double e0 = eps + d0 * d0, e1 = eps + d1 * d1;
-  const double a0 = 2.0 * e1 * e1, a1 = e0 * e0;
-  return (a0 * (0.5 * (b + c)) + a1 * (0.5 * (3.0 * b - a))) / (a0 + a1);
+  const double e0 = fma(d0, d0, eps), e1 = fma(d1, d1, eps);
+  const double t = e1 * e1;
+  const double w0 = (t + t) * fast_rcp(fma(e0, e0, t + t));
+  return fma(0.5, fma(w0, d0 - d1, d1), b);
 }
 
 }  // namespace rmhd

@@ -107,21 +107,40 @@ void resolve_events(rmhd_ctx* c) {  // stream must be synchronised
 // ---- launches ----------------------------------------------------------------------------
 template <int MODEL, int AXIS>
 int launch_flux_axis(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODEL>& wr, double* L, int accumulate) {
-  constexpr int TS = Tile<AXIS>::TS, TO = Tile<AXIS>::TO;
   static bool attr_set[8] = {false, false, false, false, false, false, false, false};
-  const size_t smem = flux_smem_bytes<MODEL, AXIS>();
-  if (!attr_set[c->device & 7]) {
-    CK(c, cudaFuncSetAttribute(k_flux<MODEL, AXIS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_set[c->device & 7] = true;
-  }
   const int nx = c->n[0], ny = c->n[1], nz = c->n[2];
   const int ns = c->n[AXIS];
-  dim3 grid;
-  if (AXIS == 0) grid = dim3((ny * nz + TO - 1) / TO, (ns + TS - 1) / TS, 1);
-  else grid = dim3((nx + TO - 1) / TO, (ns + TS - 1) / TS, AXIS == 1 ? nz : ny);
-  Timed t(c, KC_FLUX);
-  k_flux<MODEL, AXIS><<<grid, FLUX_THREADS, smem, c->stream>>>(qr, wr, L, c->N, nx, ny, nz, c->p.bc[AXIS], 1.0 / c->dx[AXIS], accumulate, c->P);
-  CK(c, cudaGetLastError());
+  if constexpr (AXIS == 0) {
+    constexpr int TS = Tile<AXIS>::TS, TO = Tile<AXIS>::TO;
+    const size_t smem = flux_smem_bytes<MODEL, AXIS>();
+    if (!attr_set[c->device & 7]) {
+      CK(c, cudaFuncSetAttribute(k_flux<MODEL, AXIS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      attr_set[c->device & 7] = true;
+    }
+    dim3 grid((ny * nz + TO - 1) / TO, (ns + TS - 1) / TS, 1);
+    Timed t(c, KC_FLUX);
+    k_flux<MODEL, AXIS><<<grid, FLUX_THREADS, smem, c->stream>>>(qr, wr, L, c->N, nx, ny, nz, c->p.bc[AXIS], 1.0 / c->dx[AXIS], accumulate, c->P);
+    CK(c, cudaGetLastError());
+  } else {
+    const size_t smem = march_smem_bytes<MODEL>();
+    if (!attr_set[c->device & 7]) {
+      CK(c, cudaFuncSetAttribute(k_flux_march<MODEL, AXIS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      attr_set[c->device & 7] = true;
+    }
+    // segments along the sweep axis: enough threads for ~8 resident waves-worth of columns, segments >= 8 cells
+    const long long columns = (long long)((nx + MARCH_THREADS - 1) / MARCH_THREADS) * MARCH_THREADS * (AXIS == 1 ? nz : ny);
+    const long long want_threads = 148LL * 384 * 4;
+    int nseg = (int)((want_threads + columns - 1) / columns);
+    if (nseg < 1) nseg = 1;
+    if (nseg > (ns + 7) / 8) nseg = (ns + 7) / 8;
+    if (nseg > 65535) nseg = 65535;
+    const int seg_len = (ns + nseg - 1) / nseg;
+    nseg = (ns + seg_len - 1) / seg_len;
+    dim3 grid((nx + MARCH_THREADS - 1) / MARCH_THREADS, AXIS == 1 ? nz : ny, nseg);
+    Timed t(c, KC_FLUX);
+    k_flux_march<MODEL, AXIS><<<grid, MARCH_THREADS, smem, c->stream>>>(qr, wr, L, c->N, nx, ny, nz, c->p.bc[AXIS], 1.0 / c->dx[AXIS], accumulate, seg_len, c->P);
+    CK(c, cudaGetLastError());
+  }
   return RMHD_OK;
 }
 
