@@ -11,7 +11,7 @@ Prints ONE JSON line (rank 0).  Multi-GPU: the path does not shard in this build
 only"): each rank steps its own copy; value = zone-updates of all ranks / max time.
 
 `--impl reference` times the CPU oracle as it stands on the host cores, on a bounded sample of
-the same workload (a 64^3 sub-box of the 256^3 initial data around the blast, one step per
+the same workload (a 96^3 sub-box of the 256^3 initial data around the blast, one step per
 "step").  The oracle is a deliberately slow checker: the ratio to it is context, not a target.
 """
 import argparse
@@ -111,11 +111,11 @@ def make_workload(name, synth):
 
 
 def oracle_sample(cfg, synth):
-    """A bounded sample of the workload for the CPU oracle: central 64^3 (or whole grid if smaller)."""
+    """A bounded sample of the workload for the CPU oracle: central 96^3 (or whole grid if smaller)."""
     p = dict(cfg["params"])
     w = cfg["prims"]
     nz, ny, nx = w.shape[1:]
-    m = 64
+    m = 96
     if nz > m and ny > m and nx > m:
         sl = [slice((n - m) // 2, (n - m) // 2 + m) for n in (nz, ny, nx)]
         dx = [(p["zlim"][1] - p["zlim"][0]) / nz, (p["ylim"][1] - p["ylim"][0]) / ny, (p["xlim"][1] - p["xlim"][0]) / nx]
@@ -295,7 +295,7 @@ def run_ours(args):
         return
     cpu_base = None
     if world == 1 and not args.no_cpu_baseline:
-        cpu_base, _, _ = time_oracle(cfg, synth, steps=2, warmup=0, budget_s=30.0)
+        cpu_base, _, _ = time_oracle(cfg, synth, steps=12, warmup=0, budget_s=20.0)
     launches = sum(v["launches"] for v in kt.values())
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
