@@ -249,6 +249,102 @@ __global__ void __launch_bounds__(128) k_stage_batch_resistive(const double* __r
 }
 
 // =======================================================================================
+// a1: implicit stage, two-fluid (same launch shape and warp-voted loop as the resistive one).
+// Source rows (Psi storage order): Sbar(3), taubar, E(3), psi, phi  = cons rows 6..9, 13..17.
+// =======================================================================================
+template <int STAGE>
+__global__ void __launch_bounds__(128) k_stage_two_fluid(const double* __restrict__ qn, const double* __restrict__ L1,
+                                                         const double* __restrict__ Ps1, double* __restrict__ w,
+                                                         double* __restrict__ qs, double* __restrict__ Ps, size_t N, double a,
+                                                         double cL, double cP, DevPar P, Stats* st) {
+  __shared__ int shist[NBINS];
+  BlockHist bh; bh.init(shist);
+  const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const bool valid = c < N;
+  TStage s;
+  s.status = 1; s.iters = 0;
+  double qpsi = 0.0, qphi = 0.0;
+  if (valid) {
+    double qe[T_NC], wg[T_NH];
+#pragma unroll
+    for (int v = 0; v < T_NC; ++v) qe[v] = qn[(size_t)v * N + c];
+    if (STAGE == 2) {
+#pragma unroll
+      for (int v = 0; v < T_NC; ++v) qe[v] += cL * L1[(size_t)v * N + c];
+#pragma unroll
+      for (int k = 0; k < T_NS; ++k) qe[k < 4 ? 6 + k : 9 + k] += cP * Ps1[(size_t)k * N + c];
+#pragma unroll
+      for (int v = 0; v < T_NC; ++v) if (v < 6 || (v >= 10 && v < 13)) qs[(size_t)v * N + c] = qe[v];
+    }
+    qpsi = qe[16]; qphi = qe[17];
+#pragma unroll
+    for (int v = 0; v < T_NH; ++v) wg[v] = w[(size_t)v * N + c];
+    t_stage_init(s, qe, wg, a, P);
+  }
+  while (true) {
+    const bool active = s.status == 0 && s.iters < P.maxit_stage;
+    if (!__any_sync(0xffffffffu, active)) break;
+    if (active) t_stage_iter(s, P);
+  }
+  if (valid) {
+    double wl[T_NH], src[T_NS], psi, phi;
+    t_stage_finish(s, P, wl, src, psi, phi, qpsi, qphi);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { qs[(size_t)(6 + i) * N + c] = s.Sb[i]; qs[(size_t)(13 + i) * N + c] = s.E[i]; }
+    qs[9 * N + c] = s.tb; qs[16 * N + c] = psi; qs[17 * N + c] = phi;
+#pragma unroll
+    for (int v = 0; v < T_NH; ++v) w[(size_t)v * N + c] = wl[v];
+#pragma unroll
+    for (int k = 0; k < T_NS; ++k) Ps[(size_t)k * N + c] = src[k];
+    bh.add(s.iters);
+    if (s.status != 1 || !(wl[0] > 0.0) || !(wl[4] > 0.0) || !(wl[5] > 0.0) || !(wl[9] > 0.0)) record_fail(st, (long long)c);
+  }
+  bh.flush(st->hist_stage);
+}
+
+// batched two-fluid implicit stage on independent cells: boundary layouts
+__global__ void __launch_bounds__(128) k_stage_batch_two_fluid(const double* __restrict__ q_ex, const double* __restrict__ prim_guess,
+                                                               double a, double* __restrict__ q_out, double* __restrict__ prims_out,
+                                                               int* __restrict__ iters, int* __restrict__ fail, size_t N, DevPar P) {
+  const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const bool valid = c < N;
+  TStage s;
+  s.status = 1; s.iters = 0;
+  double qpsi = 0.0, qphi = 0.0;
+  if (valid) {
+    double qe[T_NC], wg[T_NH];
+#pragma unroll
+    for (int v = 0; v < T_NC; ++v) qe[v] = q_ex[(size_t)v * N + c];
+#pragma unroll
+    for (int v = 0; v < T_NC; ++v) if (v < 6 || (v >= 10 && v < 13)) q_out[(size_t)v * N + c] = qe[v];
+    qpsi = qe[16]; qphi = qe[17];
+#pragma unroll
+    for (int v = 0; v < T_NH; ++v) wg[v] = prim_guess[(size_t)v * N + c];
+    t_stage_init(s, qe, wg, a, P);
+  }
+  while (true) {
+    const bool active = s.status == 0 && s.iters < P.maxit_stage;
+    if (!__any_sync(0xffffffffu, active)) break;
+    if (active) t_stage_iter(s, P);
+  }
+  if (valid) {
+    double wl[T_NH], src[T_NS], psi, phi;
+    t_stage_finish(s, P, wl, src, psi, phi, qpsi, qphi);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { q_out[(size_t)(6 + i) * N + c] = s.Sb[i]; q_out[(size_t)(13 + i) * N + c] = s.E[i]; }
+    q_out[9 * N + c] = s.tb; q_out[16 * N + c] = psi; q_out[17 * N + c] = phi;
+#pragma unroll
+    for (int v = 0; v < T_NH; ++v) prims_out[(size_t)v * N + c] = wl[v];
+    prims_out[10 * N + c] = s.Bx; prims_out[11 * N + c] = s.By; prims_out[12 * N + c] = s.Bz;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) prims_out[(size_t)(13 + i) * N + c] = s.E[i];
+    if (iters) iters[c] = s.iters;
+    const bool phys = wl[0] > 0.0 && wl[4] > 0.0 && wl[5] > 0.0 && wl[9] > 0.0;
+    if (fail) fail[c] = (s.status == 1 && phys) ? 0 : (s.status == 1 ? 3 : (s.status == 0 ? 2 : 10 - s.status));
+  }
+}
+
+// =======================================================================================
 // a4: L(q) along one axis.  Flux vector + Lax-Friedrichs split (eq 12, alpha = 1) + WENO3 +
 // face flux + divergence, one CTA per tile, the stencil staged through shared memory:
 //   phase 1  every cell of the tile + 2 halo cells per side: load q, w (boundary index map =

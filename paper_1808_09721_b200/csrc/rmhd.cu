@@ -161,26 +161,29 @@ int launch_flux(rmhd_ctx* c, const double* qa, const double* qb, bool mix, const
   return RMHD_OK;
 }
 
-int step_once_resistive(rmhd_ctx* c) {
+template <int MODEL>
+int step_once(rmhd_ctx* c) {
   const double g = 1.0 - 1.0 / sqrt(2.0);
   const double dt = c->dt;
   const unsigned nb = blocks_for(c->N, 128);
   int rc;
   {
     Timed t(c, KC_STAGE1);
-    k_stage_resistive<1><<<nb, 128, 0, c->stream>>>(c->q, nullptr, nullptr, c->w, c->qs, c->Ps1, c->N, g * dt, 0.0, 0.0, c->P, c->d_stats);
+    if (MODEL == 0) k_stage_resistive<1><<<nb, 128, 0, c->stream>>>(c->q, nullptr, nullptr, c->w, c->qs, c->Ps1, c->N, g * dt, 0.0, 0.0, c->P, c->d_stats);
+    else k_stage_two_fluid<1><<<nb, 128, 0, c->stream>>>(c->q, nullptr, nullptr, c->w, c->qs, c->Ps1, c->N, g * dt, 0.0, 0.0, c->P, c->d_stats);
     CK(c, cudaGetLastError());
   }
-  if ((rc = launch_flux<0>(c, c->q, c->qs, true, c->w, c->L1))) return rc;
+  if ((rc = launch_flux<MODEL>(c, c->q, c->qs, true, c->w, c->L1))) return rc;
   {
     Timed t(c, KC_STAGE2);
-    k_stage_resistive<2><<<nb, 128, 0, c->stream>>>(c->q, c->L1, c->Ps1, c->w, c->qs, c->Ps2, c->N, g * dt, dt, (1.0 - 2.0 * g) * dt, c->P, c->d_stats);
+    if (MODEL == 0) k_stage_resistive<2><<<nb, 128, 0, c->stream>>>(c->q, c->L1, c->Ps1, c->w, c->qs, c->Ps2, c->N, g * dt, dt, (1.0 - 2.0 * g) * dt, c->P, c->d_stats);
+    else k_stage_two_fluid<2><<<nb, 128, 0, c->stream>>>(c->q, c->L1, c->Ps1, c->w, c->qs, c->Ps2, c->N, g * dt, dt, (1.0 - 2.0 * g) * dt, c->P, c->d_stats);
     CK(c, cudaGetLastError());
   }
-  if ((rc = launch_flux<0>(c, c->qs, nullptr, false, c->w, c->L2))) return rc;
+  if ((rc = launch_flux<MODEL>(c, c->qs, nullptr, false, c->w, c->L2))) return rc;
   {
     Timed t(c, KC_FINAL);
-    k_final<0><<<blocks_for(c->N, 256), 256, 0, c->stream>>>(c->q, c->L1, c->L2, c->Ps1, c->Ps2, c->w, c->N, 0.5 * dt, c->P, c->d_stats);
+    k_final<MODEL><<<blocks_for(c->N, 256), 256, 0, c->stream>>>(c->q, c->L1, c->L2, c->Ps1, c->Ps2, c->w, c->N, 0.5 * dt, c->P, c->d_stats);
     CK(c, cudaGetLastError());
   }
   return RMHD_OK;
@@ -329,9 +332,8 @@ int rmhd_set_cons(rmhd_ctx* c, const double* cons, const double* prim_guess, int
 int rmhd_step(rmhd_ctx* c, int nsteps) {
   if (!c || nsteps < 0) return RMHD_ERR_BAD_PARAM;
   DeviceGuard dg(c->device);
-  if (c->model != 0) { c->err = "two-fluid stepping not built yet"; return RMHD_ERR_BAD_PARAM; }
   for (int s = 0; s < nsteps; ++s) {
-    int rc = step_once_resistive(c);
+    int rc = c->model == 0 ? step_once<0>(c) : step_once<1>(c);
     if (rc) return rc;
     c->nsteps++;
   }
@@ -452,12 +454,12 @@ int rmhd_stage_batch(const rmhd_params* p, long long ncells, const double* q_ex,
   int rc = batch_prologue(p, ncells, P);
   if (rc) return rc;
   if (!q_ex || !prim_guess || !q_out || !prims_out) { g_create_error = "null buffer"; return RMHD_ERR_BAD_PARAM; }
-  if (p->model != RMHD_RESISTIVE) { g_create_error = "two-fluid stage batch not built yet"; return RMHD_ERR_BAD_PARAM; }
+  if (p->model == RMHD_TWO_FLUID && sigma_cell) { g_create_error = "sigma_cell is a resistive-model argument"; return RMHD_ERR_BAD_PARAM; }
   if (ncells == 0) return RMHD_OK;
   DeviceGuard dg(p->device);
   cudaStream_t s = (cudaStream_t)p->stream;
   const size_t N = (size_t)ncells;
-  const int nc = 14, np = 11;
+  const int nc = p->model == 0 ? 14 : 18, np = p->model == 0 ? 11 : 16;
   Staging st(s);
   const double *d_qex = q_ex, *d_pg = prim_guess, *d_sig = sigma_cell;
   double *d_qo = q_out, *d_po = prims_out; int *d_it = iters, *d_fl = fail;
@@ -466,7 +468,8 @@ int rmhd_stage_batch(const rmhd_params* p, long long ncells, const double* q_ex,
     CK(nullptr, st.out(q_out, nc * N, &d_qo)); CK(nullptr, st.out(prims_out, np * N, &d_po));
     CK(nullptr, st.out(iters, N, &d_it)); CK(nullptr, st.out(fail, N, &d_fl));
   }
-  k_stage_batch_resistive<<<blocks_for(N, 128), 128, 0, s>>>(d_qex, d_pg, d_sig, a_dt, d_qo, d_po, d_it, d_fl, N, P);
+  if (p->model == 0) k_stage_batch_resistive<<<blocks_for(N, 128), 128, 0, s>>>(d_qex, d_pg, d_sig, a_dt, d_qo, d_po, d_it, d_fl, N, P);
+  else k_stage_batch_two_fluid<<<blocks_for(N, 128), 128, 0, s>>>(d_qex, d_pg, a_dt, d_qo, d_po, d_it, d_fl, N, P);
   CK(nullptr, cudaGetLastError());
   if (!on_device) {
     CK(nullptr, cudaMemcpyAsync(q_out, d_qo, sizeof(double) * nc * N, cudaMemcpyDeviceToHost, s));

@@ -171,3 +171,286 @@ RMHD_DEV void r_stage_finish(const RStage& s, const DevPar& P, Hyd& h, double* J
 }
 
 }  // namespace rmhd
+
+namespace rmhd {
+
+// ---------------------------------------------------------------------------------------
+// Two-fluid stage (A2-A3 P:L445-451, eq 7-8; readings G2, G3).  Rows with a source:
+// Sbar (3), taubar, E (3) [psi, phi closed form with rhoc = Dbar fixed]; D, S, tau, Dbar, B equal
+// q_ex.  Unknowns x = (Sbar, taubar, E) and Z_e, Z_p (one per species, replacing the two nested
+// con2prims):
+//   F_Sbar = Sbar - Sbar_ex - a [Kq E + U x B - eta (wp2 J - rho0 U)]
+//   F_tbar = tbar - tbar_ex - a [U.E - eta (wp2 rhoc - rho0 Kq)]
+//   F_E    = E - E_ex + a J
+//   G_s    = Z_s - p_s(Z_s, S_s) - tau_s - D_s,   S_s = c_s Sbar + d_s (S - E x B),
+//            tau_s = c_s tbar + d_s (tau - (E^2+B^2)/2),   v_s = S_s / Z_s
+// with m_s = mu_s D_s, m2_s = mu_s^2 D_s (constants of the stage), Kq = sum m2_s, rhoc = sum m_s,
+// J = sum m_s v_s, U = sum m2_s v_s, wp2 = sum m2_s sqrt(1-v_s^2), rho0 = (Kq rhoc - J.U)/wp2.
+// Jacobian by exact forward-mode tangents, one direction at a time (all in registers); Z_e, Z_p
+// eliminated (dG_s/dZ_t = 0 for s != t), leaving a 7x7 system solved by Gaussian elimination
+// in the order (Sbar, tbar, E): the pivots are 1 + a eta wp2 k > 0 and 1 + a^2 k Kq/(..) > 0
+// (k = sum m_s c_s / Z_s), so no pivoting is needed.
+// ---------------------------------------------------------------------------------------
+struct TKin { double iZ, vx, vy, vz, om, W, sq; };
+
+struct TStage {
+  double D[2], Sx, Sy, Sz, tau, Bx, By, Bz, B2;
+  double Sbex[3], tbex, Eex[3];
+  double m[2], m2[2], Kq, rhoc;
+  double c[2], d[2];          // species split: x_s = c_s xbar + d_s x
+  double a, eta, scale;
+  double Sb[3], tb, E[3], Z[2];
+  int status, iters;
+};
+
+// species momenta / energies at (Sb, tb, E); returns admissibility of both species for given Z
+RMHD_DEV bool t_species(const TStage& s, const double* Sb, double tb, const double* E, const double* Z,
+                        double Ss[2][3], double* ts) {
+  const double tx = s.Sx - (E[1] * s.Bz - E[2] * s.By);
+  const double ty = s.Sy - (E[2] * s.Bx - E[0] * s.Bz);
+  const double tz = s.Sz - (E[0] * s.By - E[1] * s.Bx);
+  const double taut = s.tau - 0.5 * (E[0] * E[0] + E[1] * E[1] + E[2] * E[2] + s.B2);
+  bool ok = true;
+#pragma unroll
+  for (int k = 0; k < 2; ++k) {
+    Ss[k][0] = s.c[k] * Sb[0] + s.d[k] * tx;
+    Ss[k][1] = s.c[k] * Sb[1] + s.d[k] * ty;
+    Ss[k][2] = s.c[k] * Sb[2] + s.d[k] * tz;
+    ts[k] = s.c[k] * tb + s.d[k] * taut;
+    const double S2 = Ss[k][0] * Ss[k][0] + Ss[k][1] * Ss[k][1] + Ss[k][2] * Ss[k][2];
+    const double tD = ts[k] + s.D[k];
+    ok = ok && (tD > 0.0) && (tD * tD > S2) && (Z[k] > 0.0) && (Z[k] * Z[k] > S2 * (1.0 + 1e-14));
+  }
+  return ok;
+}
+
+// q_ex: the 18 explicit-part rows; wg: 10 hydro primitives near the solution
+RMHD_DEV void t_stage_init(TStage& s, const double* qe, const double* wg, double a, const DevPar& P) {
+  const Split sp(P);
+  s.c[0] = sp.ce; s.d[0] = sp.de; s.c[1] = sp.cp; s.d[1] = sp.dp;
+  s.D[0] = sp.ce * qe[5] + sp.de * qe[0];
+  s.D[1] = sp.cp * qe[5] + sp.dp * qe[0];
+  s.Sx = qe[1]; s.Sy = qe[2]; s.Sz = qe[3]; s.tau = qe[4];
+  s.Bx = qe[10]; s.By = qe[11]; s.Bz = qe[12];
+  s.B2 = s.Bx * s.Bx + s.By * s.By + s.Bz * s.Bz;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { s.Sbex[i] = qe[6 + i]; s.Eex[i] = qe[13 + i]; s.Sb[i] = qe[6 + i]; s.E[i] = qe[13 + i]; }
+  s.tbex = qe[9]; s.tb = qe[9];
+  s.m[0] = P.mu_e * s.D[0]; s.m[1] = P.mu_p * s.D[1];
+  s.m2[0] = P.mu_e * s.m[0]; s.m2[1] = P.mu_p * s.m[1];
+  s.Kq = s.m2[0] + s.m2[1]; s.rhoc = s.m[0] + s.m[1];
+  s.a = a; s.eta = P.eta;
+  s.status = 0; s.iters = 0;
+  double sc = 1.0;
+#pragma unroll
+  for (int v = 0; v < 16; ++v) sc = fmax(sc, fabs(qe[v]));
+  s.scale = sc;
+#pragma unroll
+  for (int k = 0; k < 2; ++k) s.Z[k] = Z_of_prims(wg[5 * k], wg[5 * k + 1], wg[5 * k + 2], wg[5 * k + 3], wg[5 * k + 4], P);
+  if (!(s.D[0] > 0.0) || !(s.D[1] > 0.0) || !isfinite(sc)) { s.status = -1; return; }
+  // the guess must be admissible for both species; repair Z_s if only that is off
+  double Ss[2][3], ts[2];
+  if (!t_species(s, s.Sb, s.tb, s.E, s.Z, Ss, ts)) {
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+      const double S2 = Ss[k][0] * Ss[k][0] + Ss[k][1] * Ss[k][1] + Ss[k][2] * Ss[k][2];
+      if (!(s.Z[k] * s.Z[k] > S2 * (1.0 + 1e-14)) || !isfinite(s.Z[k])) s.Z[k] = fmax(ts[k] + s.D[k], sqrt(S2) * (1.0 + 1e-8) + 1e-300);
+    }
+    if (!t_species(s, s.Sb, s.tb, s.E, s.Z, Ss, ts)) s.status = -1;
+  }
+}
+
+// tangent of one species' kinematics: inputs (dS, dZ, dtau_s) -> dv, dsq, dG
+RMHD_DEV void t_kin_tan(const TKin& k, double Z, double D, double g, double dSx, double dSy, double dSz, double dZ, double dts,
+                        double* dv, double& dsq, double& dG) {
+  dv[0] = (dSx - k.vx * dZ) * k.iZ;
+  dv[1] = (dSy - k.vy * dZ) * k.iZ;
+  dv[2] = (dSz - k.vz * dZ) * k.iZ;
+  const double dom = -2.0 * (k.vx * dv[0] + k.vy * dv[1] + k.vz * dv[2]);
+  dsq = 0.5 * dom * k.W;
+  dG = dZ - g * (dZ * k.om + Z * dom - D * dsq) - dts;
+}
+
+struct TAgg { double J[3], U[3], wp2, iw, rho0; };
+
+// tangent of the seven F rows given the species tangents and the direct (dSb, dtb, dE) parts
+RMHD_DEV void t_F_tan(const TStage& s, const TAgg& A, const double dv[2][3], const double* dsq,
+                      const double* dSb, double dtb, const double* dE, double* dF) {
+  double dJ[3], dU[3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { dJ[i] = s.m[0] * dv[0][i] + s.m[1] * dv[1][i]; dU[i] = s.m2[0] * dv[0][i] + s.m2[1] * dv[1][i]; }
+  const double dwp2 = s.m2[0] * dsq[0] + s.m2[1] * dsq[1];
+  const double dJU = dJ[0] * A.U[0] + dJ[1] * A.U[1] + dJ[2] * A.U[2] + A.J[0] * dU[0] + A.J[1] * dU[1] + A.J[2] * dU[2];
+  const double drho0 = -(dJU + A.rho0 * dwp2) * A.iw;
+  const double E0 = s.E[0], E1 = s.E[1], E2 = s.E[2];
+  const double cx = dU[1] * s.Bz - dU[2] * s.By, cy = dU[2] * s.Bx - dU[0] * s.Bz, cz = dU[0] * s.By - dU[1] * s.Bx;
+  const double ae = s.a * s.eta;
+  dF[0] = dSb[0] - s.a * (s.Kq * dE[0] + cx) + ae * (dwp2 * A.J[0] + A.wp2 * dJ[0] - drho0 * A.U[0] - A.rho0 * dU[0]);
+  dF[1] = dSb[1] - s.a * (s.Kq * dE[1] + cy) + ae * (dwp2 * A.J[1] + A.wp2 * dJ[1] - drho0 * A.U[1] - A.rho0 * dU[1]);
+  dF[2] = dSb[2] - s.a * (s.Kq * dE[2] + cz) + ae * (dwp2 * A.J[2] + A.wp2 * dJ[2] - drho0 * A.U[2] - A.rho0 * dU[2]);
+  dF[3] = dtb - s.a * (dU[0] * E0 + dU[1] * E1 + dU[2] * E2 + A.U[0] * dE[0] + A.U[1] * dE[1] + A.U[2] * dE[2])
+          + ae * (dwp2 * s.rhoc - drho0 * s.Kq);
+  dF[4] = dE[0] + s.a * dJ[0];
+  dF[5] = dE[1] + s.a * dJ[1];
+  dF[6] = dE[2] + s.a * dJ[2];
+}
+
+RMHD_DEV void t_stage_iter(TStage& s, const DevPar& P) {
+  double Ss[2][3], ts[2];
+  t_species(s, s.Sb, s.tb, s.E, s.Z, Ss, ts);
+  TKin k[2];
+  double G[2];
+#pragma unroll
+  for (int q = 0; q < 2; ++q) {
+    k[q].iZ = 1.0 / s.Z[q];
+    k[q].vx = Ss[q][0] * k[q].iZ; k[q].vy = Ss[q][1] * k[q].iZ; k[q].vz = Ss[q][2] * k[q].iZ;
+    k[q].om = 1.0 - (k[q].vx * k[q].vx + k[q].vy * k[q].vy + k[q].vz * k[q].vz);
+    k[q].W = rsqrt(k[q].om);
+    k[q].sq = k[q].om * k[q].W;
+    G[q] = s.Z[q] - P.g * (s.Z[q] * k[q].om - s.D[q] * k[q].sq) - ts[q] - s.D[q];
+  }
+  TAgg A;
+  A.J[0] = s.m[0] * k[0].vx + s.m[1] * k[1].vx; A.J[1] = s.m[0] * k[0].vy + s.m[1] * k[1].vy; A.J[2] = s.m[0] * k[0].vz + s.m[1] * k[1].vz;
+  A.U[0] = s.m2[0] * k[0].vx + s.m2[1] * k[1].vx; A.U[1] = s.m2[0] * k[0].vy + s.m2[1] * k[1].vy; A.U[2] = s.m2[0] * k[0].vz + s.m2[1] * k[1].vz;
+  A.wp2 = s.m2[0] * k[0].sq + s.m2[1] * k[1].sq;
+  A.iw = 1.0 / A.wp2;
+  A.rho0 = (s.Kq * s.rhoc - (A.J[0] * A.U[0] + A.J[1] * A.U[1] + A.J[2] * A.U[2])) * A.iw;
+  double F[7];
+  {
+    const double ae = s.a * s.eta;
+    F[0] = s.Sb[0] - s.Sbex[0] - s.a * (s.Kq * s.E[0] + (A.U[1] * s.Bz - A.U[2] * s.By)) + ae * (A.wp2 * A.J[0] - A.rho0 * A.U[0]);
+    F[1] = s.Sb[1] - s.Sbex[1] - s.a * (s.Kq * s.E[1] + (A.U[2] * s.Bx - A.U[0] * s.Bz)) + ae * (A.wp2 * A.J[1] - A.rho0 * A.U[1]);
+    F[2] = s.Sb[2] - s.Sbex[2] - s.a * (s.Kq * s.E[2] + (A.U[0] * s.By - A.U[1] * s.Bx)) + ae * (A.wp2 * A.J[2] - A.rho0 * A.U[2]);
+    F[3] = s.tb - s.tbex - s.a * (A.U[0] * s.E[0] + A.U[1] * s.E[1] + A.U[2] * s.E[2]) + ae * (A.wp2 * s.rhoc - A.rho0 * s.Kq);
+    F[4] = s.E[0] - s.Eex[0] + s.a * A.J[0];
+    F[5] = s.E[1] - s.Eex[1] + s.a * A.J[1];
+    F[6] = s.E[2] - s.Eex[2] + s.a * A.J[2];
+  }
+  const double zero3[3] = {0.0, 0.0, 0.0};
+  // ---- Z_s directions: dF/dZ_s (7 each), dG_s/dZ_s
+  double FZ[2][7], rGZ[2];
+#pragma unroll
+  for (int q = 0; q < 2; ++q) {
+    double dv[2][3] = {{0, 0, 0}, {0, 0, 0}}, dsq[2] = {0, 0}, dG;
+    t_kin_tan(k[q], s.Z[q], s.D[q], P.g, 0.0, 0.0, 0.0, 1.0, 0.0, dv[q], dsq[q], dG);
+    t_F_tan(s, A, dv, dsq, zero3, 0.0, zero3, FZ[q]);
+    rGZ[q] = 1.0 / dG;
+  }
+  // ---- x directions; M = dF/dx - sum_s dF/dZ_s (dG_s/dx) / (dG_s/dZ_s);  GX[s][j] = dG_s/dx_j
+  double M[7][7], GX[2][7];
+#pragma unroll
+  for (int j = 0; j < 7; ++j) {
+    double dF[7], dGs[2];
+    if (j == 3) {            // taubar: only tau_s changes
+#pragma unroll
+      for (int i = 0; i < 7; ++i) dF[i] = i == 3 ? 1.0 : 0.0;
+      dGs[0] = -s.c[0]; dGs[1] = -s.c[1];
+    } else {
+      double dSb[3] = {0, 0, 0}, dE[3] = {0, 0, 0}, dSt[3] = {0, 0, 0}, dtaut = 0.0, cS = 0.0;
+      if (j < 3) { dSb[j] = 1.0; cS = 1.0; }
+      else {
+        const int e = j - 4;
+        dE[e] = 1.0;
+        // d(S - E x B)/dE_e = -(e_e x B)
+        if (e == 0) { dSt[1] = s.Bz; dSt[2] = -s.By; }
+        if (e == 1) { dSt[0] = -s.Bz; dSt[2] = s.Bx; }
+        if (e == 2) { dSt[0] = s.By; dSt[1] = -s.Bx; }
+        dtaut = -s.E[e];
+      }
+      double dv[2][3], dsq[2];
+#pragma unroll
+      for (int q = 0; q < 2; ++q)
+        t_kin_tan(k[q], s.Z[q], s.D[q], P.g, s.c[q] * cS * dSb[0] + s.d[q] * dSt[0], s.c[q] * cS * dSb[1] + s.d[q] * dSt[1],
+                  s.c[q] * cS * dSb[2] + s.d[q] * dSt[2], 0.0, s.d[q] * dtaut, dv[q], dsq[q], dGs[q]);
+      t_F_tan(s, A, dv, dsq, dSb, 0.0, dE, dF);
+    }
+    const double w0 = dGs[0] * rGZ[0], w1 = dGs[1] * rGZ[1];
+    GX[0][j] = dGs[0]; GX[1][j] = dGs[1];
+#pragma unroll
+    for (int i = 0; i < 7; ++i) M[i][j] = dF[i] - FZ[0][i] * w0 - FZ[1][i] * w1;
+  }
+  double b[7];
+  {
+    const double w0 = G[0] * rGZ[0], w1 = G[1] * rGZ[1];
+#pragma unroll
+    for (int i = 0; i < 7; ++i) b[i] = -(F[i] - FZ[0][i] * w0 - FZ[1][i] * w1);
+  }
+  // ---- Gaussian elimination, no pivoting (see header comment)
+#pragma unroll
+  for (int c = 0; c < 7; ++c) {
+    const double r = 1.0 / M[c][c];
+#pragma unroll
+    for (int i = c + 1; i < 7; ++i) {
+      const double f = M[i][c] * r;
+#pragma unroll
+      for (int j = c + 1; j < 7; ++j) M[i][j] -= f * M[c][j];
+      b[i] -= f * b[c];
+    }
+  }
+  double dx[7];
+#pragma unroll
+  for (int i = 6; i >= 0; --i) {
+    double t = b[i];
+#pragma unroll
+    for (int j = i + 1; j < 7; ++j) t -= M[i][j] * dx[j];
+    dx[i] = t / M[i][i];
+  }
+  double dZ[2];
+#pragma unroll
+  for (int q = 0; q < 2; ++q) {
+    double t = G[q];
+#pragma unroll
+    for (int j = 0; j < 7; ++j) t += GX[q][j] * dx[j];
+    dZ[q] = -t * rGZ[q];
+  }
+  s.iters++;
+  double sum = dZ[0] + dZ[1];
+#pragma unroll
+  for (int j = 0; j < 7; ++j) sum += dx[j];
+  if (!isfinite(sum)) { s.status = -2; return; }
+  // keep both species admissible: halve the update if needed
+  double lam = 1.0;
+  bool ok = false;
+  double Sbn[3], En[3], Zn[2], tbn = s.tb;
+  for (int h = 0; h < 12; ++h) {
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { Sbn[i] = s.Sb[i] + lam * dx[i]; En[i] = s.E[i] + lam * dx[4 + i]; }
+    tbn = s.tb + lam * dx[3];
+    Zn[0] = s.Z[0] + lam * dZ[0]; Zn[1] = s.Z[1] + lam * dZ[1];
+    ok = t_species(s, Sbn, tbn, En, Zn, Ss, ts);
+    if (ok) break;
+    lam *= 0.5;
+  }
+  if (!ok) { s.status = -3; return; }
+  double dmax = 0.0;
+#pragma unroll
+  for (int j = 0; j < 7; ++j) dmax = fmax(dmax, fabs(dx[j]));
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { s.Sb[i] = Sbn[i]; s.E[i] = En[i]; }
+  s.tb = tbn; s.Z[0] = Zn[0]; s.Z[1] = Zn[1];
+  if (lam == 1.0 && dmax <= P.tol_stage * s.scale && fabs(dZ[0]) <= P.tol_stage * fmax(s.scale, s.Z[0]) &&
+      fabs(dZ[1]) <= P.tol_stage * fmax(s.scale, s.Z[1]))
+    s.status = 1;
+}
+
+// primitives and the source rows at the converged state.  src: Sbar(3), tbar, E(3), psi, phi rows
+RMHD_DEV void t_stage_finish(const TStage& s, const DevPar& P, double* w /*10*/, double* src /*9*/, double& psi, double& phi,
+                             double qpsi_ex, double qphi_ex) {
+  double Ss[2][3], ts[2];
+  t_species(s, s.Sb, s.tb, s.E, s.Z, Ss, ts);
+  Hyd h[2];
+#pragma unroll
+  for (int q = 0; q < 2; ++q) {
+    hyd_from_Z(s.D[q], Ss[q][0], Ss[q][1], Ss[q][2], Ss[q][0] * Ss[q][0] + Ss[q][1] * Ss[q][1] + Ss[q][2] * Ss[q][2], s.Z[q], P.g, h[q]);
+    w[5 * q] = h[q].rho; w[5 * q + 1] = h[q].vx; w[5 * q + 2] = h[q].vy; w[5 * q + 3] = h[q].vz; w[5 * q + 4] = h[q].p;
+  }
+  const double B[3] = {s.Bx, s.By, s.Bz};
+  t_source7(s.D, h, B, s.E, P, src);
+  const double ik = 1.0 / (1.0 + s.a * P.kappa);
+  psi = (qpsi_ex + s.a * s.rhoc) * ik;
+  phi = qphi_ex * ik;
+  src[7] = s.rhoc - P.kappa * psi;
+  src[8] = -P.kappa * phi;
+}
+
+}  // namespace rmhd

@@ -143,6 +143,36 @@ def test_config2_device_buffers_and_own_prim2cons(B, O, synth):
     assert rel_l1(q.cpu().numpy()[:, ok], qo[:, ok]) <= 1e-10
 
 
+@pytest.mark.parametrize("n,mu,eta,a", [(1, 100.0, 1e-4, 2e-4), (37, 100.0, 1e-4, 2e-4), (2 ** 14 + 5, 100.0, 1e-4, 2e-4),
+                                        (4099, 1e3, 1e-2, 3e-4), (4099, 1e4, 1e-3, 3e-4), (4099, 1e3, 1.0, 3e-3),
+                                        (4099, 10.0, 0.0, 1e-2)])
+def test_two_fluid_stage_batch_parity(B, O, synth, n, mu, eta, a):
+    """Two-fluid implicit stage (7+2 unknowns on the GPU, full N=18 Newton in the oracle) on random
+    admissible states; mu = 1e3, 1e4 are the paper's stiff regimes (a wp ~ 0.3..30)."""
+    w = synth.random_two_fluid_prims(n, seed=11, vmax=0.8)
+    w[10:] *= 0.3
+    if mu >= 1e3:     # stiff: start near the quasi-neutral, drift-free, ideal-Ohm state (else most cells have no root)
+        rng = np.random.default_rng(12)
+        w[5] = w[0] * (1 + 1e-4 * rng.standard_normal(n))
+        w[6:9] = w[1:4] + 1e-4 * rng.standard_normal((3, n))
+        w[13:16] = -np.cross(w[1:4], w[10:13], axis=0) + 1e-3 * rng.standard_normal((3, n))
+    kw = dict(model=1, gamma=G43, mu_e=-mu, mu_p=mu, eta=eta)
+    P, PO = B.make_params(**kw), O.make_params(**kw)
+    q_ex = O.prim2cons(PO, w)
+    qo, wo, ito, flo = O.stage_batch(PO, q_ex, w, a)
+    q = np.empty_like(q_ex); wg = np.empty_like(w); it = np.zeros(n, np.int32); fl = np.zeros(n, np.int32)
+    B.rmhd_stage_batch(P, q_ex, w, a, q, wg, None, it, fl)
+    ok = (fl == 0) & (flo == 0)
+    assert ((fl != 0) != (flo != 0)).sum() <= max(1, 1e-3 * n), ((fl != 0).sum(), (flo != 0).sum())
+    assert ok.sum() >= 0.95 * n          # the random non-neutral case has ~3 % cells with no admissible root (both sides flag them)
+    assert rel_l1(q[:, ok], qo[:, ok]) <= 1e-10, rel_l1(q[:, ok], qo[:, ok])
+    assert rel_l1(wg[:, ok], wo[:, ok]) <= 1e-10
+    # rows without a source are copied through unchanged
+    for r in (0, 1, 2, 3, 4, 5, 10, 11, 12):
+        assert np.array_equal(q[r], q_ex[r])
+    assert it[ok].min() >= 1 and np.percentile(it[ok], 99) <= 8 and it[ok].max() <= 50
+
+
 # ------------------------------------------------------------------------------------------
 # L(q): flux-vector splitting + WENO3 + divergence, virtual ghost zones
 # ------------------------------------------------------------------------------------------
@@ -253,6 +283,43 @@ def test_config5_full_size_sampled_against_oracle(B, O, synth):
     # ... and x-mirror symmetry (B_x even): S_x odd, D even
     assert np.abs(q[0] - q[0][:, :, ::-1]).max() < 1e-11
     assert np.abs(q[1] + q[1][:, :, ::-1]).max() < 1e-11
+
+
+def test_config4_two_fluid_reduced(B, O, synth):
+    c = synth.config4(nx=64, ny=48, nsteps=50)
+    q, w, st = run_gpu(B, c)
+    qo, wo, _ = run_oracle(O, c)
+    assert st["n_failed"] == 0
+    assert rel_l1(q, qo) <= 1e-8, rel_l1(q, qo)
+    assert rel_l1(w[:10], wo[:10]) <= 1e-8
+    assert st["hist_stage"].sum() == 2 * 64 * 48 * 50
+
+
+def test_config4_full_size_sampled_against_oracle(B, O, synth):
+    """1024^2 two-fluid (BASELINE.json configs[3]), two steps; the oracle recomputes a 32^2 box with
+    8 halo cells per side (2 steps x 2 stages x 2-cell stencil) from the same initial data."""
+    c = synth.config4(nsteps=2)
+    sim = B.Rmhd(**c["params"])
+    sim.set_initial(c["prims"])
+    q0, _ = sim.get_state()
+    sim.step(2)
+    q, w = sim.get_state()
+    st = sim.stats()
+    sim.close()
+    assert st["n_failed"] == 0
+    n, lo, m, h = 1024, 300, 32, 8
+    sl = slice(lo - h, lo + m + h)
+    sub = dict(c); P = dict(c["params"]); dx = 1.0 / n
+    P.update(nx=m + 2 * h, ny=m + 2 * h, bc=(0, 0, 0), xlim=((lo - h) * dx, (lo + m + h) * dx), ylim=((lo - h) * dx, (lo + m + h) * dx))
+    sub["params"] = P
+    sub["prims"] = np.ascontiguousarray(c["prims"][:, :, sl, sl])
+    qo, wo, _ = run_oracle(O, sub, nsteps=2)
+    inner = slice(h, h + m)
+    a = q[:, :, lo:lo + m, lo:lo + m]; b = qo[:, :, inner, inner]
+    assert rel_l1(a, b) <= 1e-8, rel_l1(a, b)
+    # periodic grid: the source-free rows D, S, tau, Dbar, B are conserved to round-off
+    for r in (0, 1, 2, 4, 5, 10):
+        assert abs(q[r].sum() - q0[r].sum()) <= 1e-11 * max(np.abs(q0[r]).sum(), 1.0), r
 
 
 # ------------------------------------------------------------------------------------------
