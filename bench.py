@@ -105,6 +105,10 @@ def make_workload(name, synth):
         return synth.config3()
     if name == "cfg1":
         return synth.config1()
+    if name == "cfg3_big":          # same recipe at 4096^2 = 2^24 cells (kernel studies; not a BASELINE config)
+        return synth.config3(nx=4096, ny=4096)
+    if name == "cfg4":
+        return synth.config4()
     if name == "cfg5_small":
         return synth.config5(n=64)
     raise SystemExit(f"unknown workload {name}")

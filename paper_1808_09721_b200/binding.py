@@ -21,7 +21,7 @@ NPRIM = {0: 11, 1: 16}
 KERNEL_CLASSES = ("stage1", "stage2", "flux", "combine_c2p", "other")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "librmhd.so")
+LIB_PATH = os.environ.get("RMHD_LIB") or os.path.join(_HERE, "librmhd.so")   # RMHD_LIB: an alternative build of the same library
 
 EXPORTS = (
     "rmhd_create", "rmhd_set_initial", "rmhd_set_cons", "rmhd_step", "rmhd_get_state", "rmhd_flux_divergence",

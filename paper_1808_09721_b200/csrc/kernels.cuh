@@ -24,6 +24,10 @@ __device__ __forceinline__ int bc_map(int c, int n, int bc) {
   return c < 0 ? 0 : (c >= n ? n - 1 : c);
 }
 
+// L2 prefetch of the line holding *p (no register, no scoreboard: hides DRAM latency for loads that
+// ptxas sinks next to their first use when registers are short)
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 __device__ __forceinline__ void record_fail(Stats* st, long long cell) {
   atomicAdd(&st->n_failed, 1ULL);
   atomicMin(&st->first_failed, cell);
@@ -358,6 +362,7 @@ __global__ void __launch_bounds__(128) k_stage_batch_two_fluid(const double* __r
 template <int AXIS> struct Tile { static constexpr int TS = 8, TO = 32; };
 template <> struct Tile<0> { static constexpr int TS = 64, TO = 4; };
 constexpr int FLUX_THREADS = 288;
+constexpr int FLUX_PREFETCH_CTAS = 148 * 2 + 24;   // resident CTAs (2 per SM) plus a margin
 
 template <int MODEL, int AXIS>
 constexpr size_t flux_smem_bytes() { return sizeof(double) * 2 * Dim<MODEL>::NC * (Tile<AXIS>::TS + 4) * Tile<AXIS>::TO; }
@@ -378,6 +383,21 @@ __global__ void __launch_bounds__(FLUX_THREADS, 2) k_flux(ConsRows<MODEL> qin, H
   const int s0 = blockIdx.y * TS;
   const int third = blockIdx.z;
 
+  // ---- L2 prefetch of the tile that the CTA about one wave behind this one will stage (AXIS 0 only)
+  if (AXIS == 0) {
+    const long long lin = (long long)blockIdx.x + (long long)gridDim.x * blockIdx.y + FLUX_PREFETCH_CTAS;
+    if (lin < (long long)gridDim.x * gridDim.y && tid < CS) {
+      const int pbx = (int)(lin % gridDim.x), pby = (int)(lin / gridDim.x);
+      const int c = pby * TS - 2 + tid % (TS + 4), oo = pbx * TO + tid / (TS + 4);
+      if (c < ns + 2 && oo < no) {
+        const size_t idx = (size_t)oo * nx + bc_map(c, ns, bc);
+#pragma unroll
+        for (int v = 0; v < NC; ++v) prefetch_l2(qin.r[v] + idx);
+#pragma unroll
+        for (int v = 0; v < NH; ++v) prefetch_l2(win.r[v] + idx);
+      }
+    }
+  }
   // ---- phase 1
   for (int item = tid; item < CS; item += FLUX_THREADS) {
     int sh, o;
@@ -413,12 +433,7 @@ __global__ void __launch_bounds__(FLUX_THREADS, 2) k_flux(ConsRows<MODEL> qin, H
     if (AXIS == 0) { fs = tid % (TS + 1); o = tid / (TS + 1); st = 1; }
     else { o = tid % TO; fs = tid / TO; st = TO; }
     const int base = AXIS == 0 ? o * (TS + 4) + fs : fs * TO + o;   // halo coordinate fs
-#pragma unroll
-    for (int v = 0; v < NC; ++v) {
-      const double* fp = sm + v * CS + base;
-      const double* fm = sm + (NC + v) * CS + base;
-      F[v] = weno3(fp[0], fp[st], fp[2 * st]) + weno3(fm[3 * st], fm[2 * st], fm[st]);
-    }
+    weno_faces<NC>(sm + base, sm + NC * CS + base, CS, st, F);
   }
   __syncthreads();
   if (has_face) {
@@ -520,6 +535,18 @@ k_flux_march(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, si
     for (int v = 0; v < NH; ++v) wc[v] = wn_[v];
     const bool emit = c >= s_begin + 2;
     const size_t oidx = base + (size_t)(emit ? c - 2 : 0) * stride;
+    if (c + 2 <= s_end + 1) {   // L2 prefetch of the inputs of step c + 1 (cell c + 2) and of the partial L it adds to
+      const size_t pidx = base + (size_t)bc_map(c + 2, ns, bc) * stride;
+#pragma unroll
+      for (int v = 0; v < NC; ++v) prefetch_l2(qin.r[v] + pidx);
+#pragma unroll
+      for (int v = 0; v < NH; ++v) prefetch_l2(win.r[v] + pidx);
+      if (accumulate && c < s_end) {
+        const size_t lidx = base + (size_t)(c - 1) * stride;
+#pragma unroll
+        for (int v = 0; v < NC; ++v) prefetch_l2(L + (size_t)v * N + lidx);
+      }
+    }
     // issue every global load of this step up front: next cell's inputs and the partial L to add to
     if (c <= s_end) load(c + 1, qn_, wn_);
     if (accumulate && emit) {
@@ -532,14 +559,29 @@ k_flux_march(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, si
     double f[NC];
     if (MODEL == 0) r_flux<AXIS>(qc, wc, P.sigma, P, f); else t_flux<AXIS>(qc, wc, P, f);
 #pragma unroll
-    for (int v = 0; v < NC; ++v) {
-      const double fpc = 0.5 * (f[v] + qc[v]);
-      const double fmc = 0.5 * (f[v] - qc[v]);
-      const double F = weno3(ring[a0 + v * T], ring[a1 + v * T], ring[a2 + v * T]) + weno3(fmc, ring[b1 + v * T], ring[b0 + v * T]);
-      if (emit) L[(size_t)v * N + oidx] = La[v] - (F - Fp[v]) * inv_dx;
-      Fp[v] = F;
-      ring[a0 + v * T] = fpc;
-      ring[b0 + v * T] = fmc;
+    for (int v0 = 0; v0 < NC; v0 += 4) {      // 4 variables = 8 reconstructions in flight (weno3_batch)
+      constexpr int G = 4;
+      double a[2 * G], b[2 * G], cc[2 * G], o[2 * G], fpc[G], fmc[G];
+#pragma unroll
+      for (int g = 0; g < G; ++g) {
+        const int v = v0 + g < NC ? v0 + g : NC - 1;
+        fpc[g] = 0.5 * (f[v] + qc[v]);
+        fmc[g] = 0.5 * (f[v] - qc[v]);
+        a[2 * g] = ring[a0 + v * T]; b[2 * g] = ring[a1 + v * T]; cc[2 * g] = ring[a2 + v * T];
+        a[2 * g + 1] = fmc[g]; b[2 * g + 1] = ring[b1 + v * T]; cc[2 * g + 1] = ring[b0 + v * T];
+      }
+      weno3_batch<2 * G>(a, b, cc, o);
+#pragma unroll
+      for (int g = 0; g < G; ++g) {
+        const int v = v0 + g;
+        if (v < NC) {
+          const double F = o[2 * g] + o[2 * g + 1];
+          if (emit) L[(size_t)v * N + oidx] = La[v] - (F - Fp[v]) * inv_dx;
+          Fp[v] = F;
+          ring[a0 + v * T] = fpc[g];
+          ring[b0 + v * T] = fmc[g];
+        }
+      }
     }
     { const int t = a0; a0 = a1; a1 = a2; a2 = t; }
     { const int t = b0; b0 = b1; b1 = t; }

@@ -276,21 +276,20 @@ RMHD_DEV void t_source7(const double* De /*D_e, D_p*/, const Hyd* h, const doubl
 // WENO3 (Shu 1997, r = 2; G7): value at the face between b and c biased to a.
 //   beta0 = (c-b)^2, beta1 = (b-a)^2, alpha0 = (2/3)/(eps+beta0)^2, alpha1 = (1/3)/(eps+beta1)^2
 //   u = (alpha0 (b+c)/2 + alpha1 (3b-a)/2)/(alpha0+alpha1) = b + ( d1 + w0 (d0 - d1) )/2,
-//   w0 = alpha0/(alpha0+alpha1) = 2 e1^2 / (2 e1^2 + e0^2),  e_k = eps + beta_k
-// One reciprocal per reconstruction: MUFU seed (rcp.approx.ftz.f64, ~2^-23) + 3 Newton steps
-// (full double accuracy; the denominator is >= eps^2 = 1e-12, never denormal).
+//   w0 = alpha0/(alpha0+alpha1) = e1^2 / (e1^2 + e0^2/2),  e_k = eps + beta_k,  d0 = c-b, d1 = b-a
+// One reciprocal per reconstruction: MUFU seed r0 (rcp.approx.ftz.f64 reads only the high word
+// of its input: relative error e <= ~2^-20) + one cubic step r = r0 (1 + e + e^2), error e^3
+// <= 2^-60 (the denominator is >= eps^2 = 1e-12, never denormal).  14 FP64 instructions.
+//
+// The FP64 pipe of sm_100 issues one warp instruction per 2 cycles per SM sub-partition but has
+// ~18 cycles of dependent latency (measured: utilisation = warps x ILP x 2 / 18 in profiles/r1a),
+// and ptxas emits each reconstruction as one serial chain.  weno3_batch therefore runs G
+// independent reconstructions in OPERATION-MAJOR order, so G chains are in flight per warp.
 // ---------------------------------------------------------------------------------------
-RMHD_DEV double fast_rcp(double x) {
-#ifdef __CUDA_ARCH__
+RMHD_DEV double rcp_seed(double x) {
   double r;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-  double e = fma(-x, r, 1.0); r = fma(r, e, r);
-  e = fma(-x, r, 1.0); r = fma(r, e, r);
-  e = fma(-x, r, 1.0); r = fma(r, e, r);
   return r;
-#else
-  return 1.0 / x;
-#endif
 }
 
 RMHD_DEV double weno3(double a, double b, double c) {
@@ -298,8 +297,68 @@ RMHD_DEV double weno3(double a, double b, double c) {
   const double d0 = c - b, d1 = b - a;
   const double e0 = fma(d0, d0, eps), e1 = fma(d1, d1, eps);
   const double t = e1 * e1;
-  const double w0 = (t + t) * fast_rcp(fma(e0, e0, t + t));
-  return fma(0.5, fma(w0, d0 - d1, d1), b);
+  const double den = fma(0.5 * e0, e0, t);
+  const double r0 = rcp_seed(den);
+  const double er = fma(-den, r0, 1.0);
+  const double r = fma(r0, fma(er, er, er), r0);
+  return fma(0.5, fma(t * r, d0 - d1, d1), b);
+}
+
+#ifndef RMHD_WENO_GV
+#define RMHD_WENO_GV 4   // variables per batch: 2 x RMHD_WENO_GV reconstructions in flight
+#endif
+
+template <int G>
+RMHD_DEV void weno3_batch(const double* a, const double* b, const double* c, double* out) {
+  const double eps = 1e-6;
+  double d0[G], d1[G], e0[G], e1[G], t[G], den[G], r0[G], er[G];
+#pragma unroll
+  for (int g = 0; g < G; ++g) d0[g] = c[g] - b[g];
+#pragma unroll
+  for (int g = 0; g < G; ++g) d1[g] = b[g] - a[g];
+#pragma unroll
+  for (int g = 0; g < G; ++g) e0[g] = fma(d0[g], d0[g], eps);
+#pragma unroll
+  for (int g = 0; g < G; ++g) e1[g] = fma(d1[g], d1[g], eps);
+#pragma unroll
+  for (int g = 0; g < G; ++g) t[g] = e1[g] * e1[g];
+#pragma unroll
+  for (int g = 0; g < G; ++g) e1[g] = 0.5 * e0[g];
+#pragma unroll
+  for (int g = 0; g < G; ++g) den[g] = fma(e1[g], e0[g], t[g]);
+#pragma unroll
+  for (int g = 0; g < G; ++g) r0[g] = rcp_seed(den[g]);
+#pragma unroll
+  for (int g = 0; g < G; ++g) er[g] = fma(-den[g], r0[g], 1.0);
+#pragma unroll
+  for (int g = 0; g < G; ++g) d0[g] = d0[g] - d1[g];
+#pragma unroll
+  for (int g = 0; g < G; ++g) er[g] = fma(er[g], er[g], er[g]);
+#pragma unroll
+  for (int g = 0; g < G; ++g) r0[g] = fma(r0[g], er[g], r0[g]);
+#pragma unroll
+  for (int g = 0; g < G; ++g) t[g] = t[g] * r0[g];
+#pragma unroll
+  for (int g = 0; g < G; ++g) d1[g] = fma(t[g], d0[g], d1[g]);
+#pragma unroll
+  for (int g = 0; g < G; ++g) out[g] = fma(0.5, d1[g], b[g]);
+}
+
+// face fluxes F_v = weno3(f+ at p, p+st, p+2st) + weno3(f- at m+3st, m+2st, m+st) for NV variables
+// whose f+ / f- planes are vstride apart, in groups of <= 4 variables (8 chains in flight)
+template <int NV>
+RMHD_DEV void weno_faces(const double* pp, const double* pm, int vstride, int st, double* F) {
+  constexpr int GV = NV >= RMHD_WENO_GV ? RMHD_WENO_GV : NV;
+  double a[2 * GV], b[2 * GV], c[2 * GV], o[2 * GV];
+#pragma unroll
+  for (int v = 0; v < GV; ++v) {
+    a[2 * v] = pp[v * vstride]; b[2 * v] = pp[v * vstride + st]; c[2 * v] = pp[v * vstride + 2 * st];
+    a[2 * v + 1] = pm[v * vstride + 3 * st]; b[2 * v + 1] = pm[v * vstride + 2 * st]; c[2 * v + 1] = pm[v * vstride + st];
+  }
+  weno3_batch<2 * GV>(a, b, c, o);
+#pragma unroll
+  for (int v = 0; v < GV; ++v) F[v] = o[2 * v] + o[2 * v + 1];
+  if constexpr (NV > GV) weno_faces<NV - GV>(pp + GV * vstride, pm + GV * vstride, vstride, st, F + GV);
 }
 
 }  // namespace rmhd

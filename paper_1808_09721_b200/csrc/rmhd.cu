@@ -3,11 +3,13 @@
 
 #include <climits>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
 
 #include "kernels.cuh"
+#include "flux3.cuh"
 
 using namespace rmhd;
 
@@ -35,6 +37,7 @@ struct rmhd_ctx {
   Stats* d_stats;
   Stats* h_stats;  // pinned
   bool profiling;
+  bool fused_flux;   // RMHD_FLUX=fused selects the experimental one-pass L(q) (flux3.cuh); default: per-axis kernels
   std::vector<EvRec> pending;
   std::vector<cudaEvent_t> ev_pool;
   double ms[KC_N];
@@ -144,6 +147,34 @@ int launch_flux_axis(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODEL
   return RMHD_OK;
 }
 
+// all present axes in one pass (flux3.cuh); needs nx > 1 and ny > 1
+template <int MODEL, bool HAS_Z>
+int launch_flux3(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODEL>& wr, double* L) {
+  static bool attr_set[8] = {false, false, false, false, false, false, false, false};
+  const int nx = c->n[0], ny = c->n[1], nz = c->n[2];
+  const size_t smem = F3<MODEL>::bytes(HAS_Z);
+  if (!attr_set[c->device & 7]) {
+    CK(c, cudaFuncSetAttribute(k_flux3<MODEL, HAS_Z>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr_set[c->device & 7] = true;
+  }
+  const int gx = (nx + F3_TX - 1) / F3_TX, gy = (ny + F3_TY - 1) / F3_TY;
+  int nseg = 1, seg_len = 1;
+  if (HAS_Z) {   // z segments: enough CTAs for ~6 full waves of 2 CTAs/SM, segments of >= 16 planes
+    const long long want = 148LL * 2 * 6;
+    nseg = (int)((want + (long long)gx * gy - 1) / ((long long)gx * gy));
+    if (nseg > (nz + 15) / 16) nseg = (nz + 15) / 16;
+    if (nseg < 1) nseg = 1;
+    seg_len = (nz + nseg - 1) / nseg;
+    nseg = (nz + seg_len - 1) / seg_len;
+  }
+  dim3 grid(gx, gy, nseg);
+  Timed t(c, KC_FLUX);
+  k_flux3<MODEL, HAS_Z><<<grid, F3_THREADS, smem, c->stream>>>(qr, wr, L, c->N, nx, ny, nz, c->p.bc[0], c->p.bc[1], c->p.bc[2],
+                                                            1.0 / c->dx[0], 1.0 / c->dx[1], 1.0 / c->dx[2], seg_len, c->P);
+  CK(c, cudaGetLastError());
+  return RMHD_OK;
+}
+
 // L(q) with the conserved rows taken from `qa` except the rows listed in src rows, which come
 // from `qb` when mix != 0 (stage 1 only rewrites the rows that have a source).
 template <int MODEL>
@@ -153,6 +184,7 @@ int launch_flux(rmhd_ctx* c, const double* qa, const double* qb, bool mix, const
   for (int v = 0; v < NC; ++v) qr.r[v] = qa + (size_t)v * c->N;
   if (mix) for (int k = 0; k < NS; ++k) { int v = MODEL == 0 ? (k < 3 ? 8 + k : 9 + k) : (k < 4 ? 6 + k : 9 + k); qr.r[v] = qb + (size_t)v * c->N; }
   for (int v = 0; v < NH; ++v) wr.r[v] = w + (size_t)v * c->N;
+  if (c->fused_flux && c->n[0] > 1 && c->n[1] > 1) return c->n[2] > 1 ? launch_flux3<MODEL, true>(c, qr, wr, L) : launch_flux3<MODEL, false>(c, qr, wr, L);
   int acc = 0, rc;
   if (c->n[0] > 1) { if ((rc = launch_flux_axis<MODEL, 0>(c, qr, wr, L, acc))) return rc; acc = 1; }
   if (c->n[1] > 1) { if ((rc = launch_flux_axis<MODEL, 1>(c, qr, wr, L, acc))) return rc; acc = 1; }
@@ -240,6 +272,7 @@ int rmhd_create(const rmhd_params* p, rmhd_ctx** out) {
   c->dt = inv > 0.0 ? p->cfl / inv : p->cfl;   // G9
   c->nsteps = 0; c->device = p->device; c->stream = (cudaStream_t)p->stream;
   c->profiling = false;
+  { const char* e = getenv("RMHD_FLUX"); c->fused_flux = e && strcmp(e, "fused") == 0; }
   for (int i = 0; i < KC_N; ++i) { c->ms[i] = 0.0; c->launches[i] = 0; }
   c->q = c->w = c->qs = c->L1 = c->L2 = c->Ps1 = c->Ps2 = nullptr; c->d_stats = nullptr; c->h_stats = nullptr;
   DeviceGuard dg(c->device);
