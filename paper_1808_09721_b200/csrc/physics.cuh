@@ -308,9 +308,11 @@ RMHD_DEV double weno3(double a, double b, double c) {
 #define RMHD_WENO_GV 4   // variables per batch: 2 x RMHD_WENO_GV reconstructions in flight
 #endif
 
-template <int G>
+// UNSCALED: the inputs are g+- = f +- q = 2 f+-; eps is scaled by 4 (exactly, a power of two) so the
+// nonlinear weights are bit-identical to those of the scaled data and the result is exactly twice as large.
+template <int G, bool UNSCALED = false>
 RMHD_DEV void weno3_batch(const double* a, const double* b, const double* c, double* out) {
-  const double eps = 1e-6;
+  const double eps = UNSCALED ? 4.0 * 1e-6 : 1e-6;
   double d0[G], d1[G], e0[G], e1[G], t[G], den[G], r0[G], er[G];
 #pragma unroll
   for (int g = 0; g < G; ++g) d0[g] = c[g] - b[g];

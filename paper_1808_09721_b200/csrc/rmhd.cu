@@ -9,7 +9,7 @@
 #include <vector>
 
 #include "kernels.cuh"
-#include "flux3.cuh"
+#include "flux_fused.cuh"
 
 using namespace rmhd;
 
@@ -37,7 +37,8 @@ struct rmhd_ctx {
   Stats* d_stats;
   Stats* h_stats;  // pinned
   bool profiling;
-  bool fused_flux;   // RMHD_FLUX=fused selects the experimental one-pass L(q) (flux3.cuh); default: per-axis kernels
+  bool fused_flux;   // one-pass L(q) over all axes (flux_fused.cuh) when nx, ny > 1; RMHD_FLUX=split forces the per-axis kernels
+  int sm_count;
   std::vector<EvRec> pending;
   std::vector<cudaEvent_t> ev_pool;
   double ms[KC_N];
@@ -147,30 +148,34 @@ int launch_flux_axis(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODEL
   return RMHD_OK;
 }
 
-// all present axes in one pass (flux3.cuh); needs nx > 1 and ny > 1
+// all present axes in one pass (flux_fused.cuh); needs nx > 1 and ny > 1
 template <int MODEL, bool HAS_Z>
-int launch_flux3(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODEL>& wr, double* L) {
+int launch_flux_fused(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODEL>& wr, double* L) {
   static bool attr_set[8] = {false, false, false, false, false, false, false, false};
   const int nx = c->n[0], ny = c->n[1], nz = c->n[2];
-  const size_t smem = F3<MODEL>::bytes(HAS_Z);
+  const size_t smem = FFSmem<MODEL>::bytes(HAS_Z);
   if (!attr_set[c->device & 7]) {
-    CK(c, cudaFuncSetAttribute(k_flux3<MODEL, HAS_Z>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CK(c, cudaFuncSetAttribute(k_flux_fused<MODEL, HAS_Z>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     attr_set[c->device & 7] = true;
   }
-  const int gx = (nx + F3_TX - 1) / F3_TX, gy = (ny + F3_TY - 1) / F3_TY;
+  const int gx = (nx + FF_TX - 1) / FF_TX, gy = (ny + FF_TY - 1) / FF_TY;
   int nseg = 1, seg_len = 1;
-  if (HAS_Z) {   // z segments: enough CTAs for ~6 full waves of 2 CTAs/SM, segments of >= 16 planes
-    const long long want = 148LL * 2 * 6;
-    nseg = (int)((want + (long long)gx * gy - 1) / ((long long)gx * gy));
-    if (nseg > (nz + 15) / 16) nseg = (nz + 15) / 16;
-    if (nseg < 1) nseg = 1;
-    seg_len = (nz + nseg - 1) / nseg;
-    nseg = (nz + seg_len - 1) / seg_len;
+  if (HAS_Z) {
+    // z segments: pick the count (segments of >= 16 planes) that wastes least, counting the partially filled
+    // last wave of resident CTAs (2 per SM) and the 4 feed-only prologue planes of every segment
+    const long long tiles = (long long)gx * gy, slots = 2LL * c->sm_count;
+    double best = 1e300;
+    for (int s = 1; s <= (nz + 15) / 16 && s <= 64; ++s) {
+      const int len = (nz + s - 1) / s, cnt = (nz + len - 1) / len;
+      const long long ctas = tiles * cnt, waves = (ctas + slots - 1) / slots;
+      const double cost = (double)waves * slots / (double)ctas * (1.0 + 3.0 / len);
+      if (cost < best - 1e-9) { best = cost; nseg = cnt; seg_len = len; }
+    }
   }
   dim3 grid(gx, gy, nseg);
   Timed t(c, KC_FLUX);
-  k_flux3<MODEL, HAS_Z><<<grid, F3_THREADS, smem, c->stream>>>(qr, wr, L, c->N, nx, ny, nz, c->p.bc[0], c->p.bc[1], c->p.bc[2],
-                                                            1.0 / c->dx[0], 1.0 / c->dx[1], 1.0 / c->dx[2], seg_len, c->P);
+  k_flux_fused<MODEL, HAS_Z><<<grid, FF_THREADS, smem, c->stream>>>(qr, wr, L, c->N, nx, ny, nz, c->p.bc[0], c->p.bc[1], c->p.bc[2],
+                                                                   0.5 / c->dx[0], 0.5 / c->dx[1], 0.5 / c->dx[2], seg_len, c->P);
   CK(c, cudaGetLastError());
   return RMHD_OK;
 }
@@ -184,7 +189,7 @@ int launch_flux(rmhd_ctx* c, const double* qa, const double* qb, bool mix, const
   for (int v = 0; v < NC; ++v) qr.r[v] = qa + (size_t)v * c->N;
   if (mix) for (int k = 0; k < NS; ++k) { int v = MODEL == 0 ? (k < 3 ? 8 + k : 9 + k) : (k < 4 ? 6 + k : 9 + k); qr.r[v] = qb + (size_t)v * c->N; }
   for (int v = 0; v < NH; ++v) wr.r[v] = w + (size_t)v * c->N;
-  if (c->fused_flux && c->n[0] > 1 && c->n[1] > 1) return c->n[2] > 1 ? launch_flux3<MODEL, true>(c, qr, wr, L) : launch_flux3<MODEL, false>(c, qr, wr, L);
+  if (c->fused_flux && c->n[0] > 1 && c->n[1] > 1) return c->n[2] > 1 ? launch_flux_fused<MODEL, true>(c, qr, wr, L) : launch_flux_fused<MODEL, false>(c, qr, wr, L);
   int acc = 0, rc;
   if (c->n[0] > 1) { if ((rc = launch_flux_axis<MODEL, 0>(c, qr, wr, L, acc))) return rc; acc = 1; }
   if (c->n[1] > 1) { if ((rc = launch_flux_axis<MODEL, 1>(c, qr, wr, L, acc))) return rc; acc = 1; }
@@ -272,10 +277,12 @@ int rmhd_create(const rmhd_params* p, rmhd_ctx** out) {
   c->dt = inv > 0.0 ? p->cfl / inv : p->cfl;   // G9
   c->nsteps = 0; c->device = p->device; c->stream = (cudaStream_t)p->stream;
   c->profiling = false;
-  { const char* e = getenv("RMHD_FLUX"); c->fused_flux = e && strcmp(e, "fused") == 0; }
+  { const char* e = getenv("RMHD_FLUX"); c->fused_flux = !(e && strcmp(e, "split") == 0); }
+  c->sm_count = 148;
   for (int i = 0; i < KC_N; ++i) { c->ms[i] = 0.0; c->launches[i] = 0; }
   c->q = c->w = c->qs = c->L1 = c->L2 = c->Ps1 = c->Ps2 = nullptr; c->d_stats = nullptr; c->h_stats = nullptr;
   DeviceGuard dg(c->device);
+  { int n = 0; if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, c->device) == cudaSuccess && n > 0) c->sm_count = n; }
   const size_t rows = (size_t)(4 * c->nc + c->nh + 2 * c->ns);
   cudaError_t e = cudaMalloc(&c->q, sizeof(double) * rows * c->N);
   if (e == cudaSuccess) e = cudaMalloc(&c->d_stats, sizeof(Stats));

@@ -192,6 +192,7 @@ def _random_state(model, shape, seed):
 @pytest.mark.parametrize("model,shape,bc", [
     (0, (1, 1, 67), (0, 0, 0)), (0, (1, 1, 130), (1, 1, 1)), (0, (1, 9, 70), (1, 0, 0)), (0, (1, 33, 5), (0, 1, 0)),
     (0, (7, 10, 35), (0, 1, 0)), (0, (11, 3, 66), (1, 0, 1)), (0, (9, 1, 40), (0, 0, 1)),
+    (0, (37, 6, 33), (1, 1, 1)), (0, (50, 5, 40), (0, 0, 0)), (0, (2, 2, 2), (1, 0, 1)), (1, (35, 6, 33), (0, 1, 1)),
     (1, (1, 1, 67), (1, 0, 0)), (1, (1, 12, 37), (0, 1, 0)), (1, (6, 9, 34), (1, 1, 0)),
 ])
 def test_flux_divergence_parity(B, O, model, shape, bc):
