@@ -1,0 +1,326 @@
+// flux_hm.cuh -- a4 fused, resistive model: the one-pass L(q) of flux_fused.cuh (same fields, same tile,
+// same shared-memory exchange, same two barriers per plane) with the work of every column split between
+// TWO threads by field group, so that 16 warps per SM are resident at 128 registers instead of 10 at 168:
+//   role H (warps 0-3): the 6 rows with a non-trivial flux (D, S, tau, rho_charge): 12 fields per axis.
+//                       Loads q, w of its cell, flux vectors along x, y (plane k) and z (feed plane k+2),
+//                       hydro z-ring in shared memory, stores its 6 rows of L.
+//   role M (warps 4-7): the 8 Maxwell / cleaning rows (B, E, psi, phi): 8 fields per axis, rebuilt from the
+//                       B, E, psi, phi rows for x, y, z; stores its 8 rows of L.  Because this role is the
+//                       lighter one it also takes the cells that do not divide by 128: the y-halo rows
+//                       (all 20 fields along y) and, warp 7, the 16 x-halo cells (all 20 fields along x).
+// The 5th row of y-faces is an extra pass of warp 0 of each role, the 33rd x-face of every row an extra pass
+// of lanes 0-3 of warp 1 of each role.  Each thread accumulates and stores only its own rows, so the two
+// roles never exchange L.  See flux_fused.cuh for the field definitions and the z schedule.
+#pragma once
+#include "flux_fused.cuh"
+
+namespace rmhd {
+
+constexpr int HM_THREADS = 2 * FF_MAIN;
+
+// CTA-wide barrier reached from role-specific code paths (every thread executes the same number of them)
+RMHD_DEV void hm_barrier() { asm volatile("bar.sync 1, %0;" ::"n"(HM_THREADS) : "memory"); }
+
+// reconstructions of NREC consecutive fields starting at field F0 of one face (shared memory), G at a time
+template <int F0, int NREC, int G, int DONE = 0>
+RMHD_DEV void face_recon_range(const double* p, int fs, int st, double* o) {
+  constexpr int B = NREC - DONE >= G ? G : NREC - DONE;
+  double a[B], b[B], c[B];
+#pragma unroll
+  for (int g = 0; g < B; ++g) {
+    const int f = F0 + DONE + g;
+    const double* pf = p + f * fs;
+    if (field_is_plus<0>(f)) { a[g] = pf[0]; b[g] = pf[st]; c[g] = pf[2 * st]; }
+    else { a[g] = pf[3 * st]; b[g] = pf[2 * st]; c[g] = pf[st]; }
+  }
+  weno3_batch<B, true>(a, b, c, o + DONE);
+  if constexpr (DONE + B < NREC) face_recon_range<F0, NREC, G, DONE + B>(p, fs, st, o);
+}
+
+// G of the 8 Maxwell rows in the fixed order (Bx, By, Bz, Ex, Ey, Ez, psi, phi) from P1..P4, M1..M4 of axis K
+template <int K>
+RMHD_DEV void assemble_M(const double* p, double* G) {
+  constexpr int a = (K + 1) % 3, b = (K + 2) % 3;
+  G[a] = p[0] - p[4];
+  G[3 + b] = -(p[0] + p[4]);
+  G[b] = p[1] + p[5];
+  G[3 + a] = p[1] - p[5];
+  G[K] = p[2] + p[6];
+  G[7] = p[2] - p[6];
+  G[3 + K] = p[3] + p[7];
+  G[6] = p[3] - p[7];
+}
+__host__ __device__ constexpr int hm_mrow(int m) { return m < 6 ? 5 + m : (m == 6 ? 12 : 13); }   // conserved row of Maxwell slot m
+
+#ifndef RMHD_HM_GH
+#define RMHD_HM_GH 6     // reconstructions in flight per batch, role H (12 per face)
+#endif
+
+template <bool HAS_Z>
+__global__ void __launch_bounds__(HM_THREADS, 2)
+k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int nx, int ny, int nz, int bcx, int bcy, int bcz,
+          double hidx, double hidy, double hidz, int seg_len, DevPar P) {
+  using FS = FSet<0>;
+  using SM = FFSmem<0>;
+  constexpr int NC = R_NC, NH = R_NH, NF = FS::NF, NHV = FS::NHV, NM = 8;
+  constexpr int TX = FF_TX, TY = FF_TY, XW = FF_XW, YR = FF_YR;
+  constexpr int FSX = TY * XW, FSY = YR * TX;       // field strides of gX, gY
+  extern __shared__ double sm[];
+  double* gX = sm;
+  double* gY = gX + SM::GX;
+  double* fY = gY + SM::GY;
+  double* fX = fY + SM::FY;
+  const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
+  const bool roleH = wrp < TY;
+  const int ty = wrp & (TY - 1);
+  double* ring = fX + SM::FX + (tid & (FF_MAIN - 1));   // role H only
+  const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
+  const int i = i0 + lane, j = j0 + ty;
+  const bool inside = i < nx && j < ny;
+  const int im = bc_map(i, nx, bcx), jm = bc_map(j, ny, bcy);
+  const int hrow = ty < 2 ? ty : ty + 4;              // gY row of the y-halo cell of this M thread
+  const int jh = bc_map(j0 + hrow - 2, ny, bcy);
+  const int xh_row = (lane >> 2) & 3, xh_col = (lane & 3) < 2 ? (lane & 3) : (lane & 3) + 32;
+  const int ixh = bc_map(i0 + xh_col - 2, nx, bcx), jxh = bc_map(j0 + xh_row, ny, bcy);
+  const size_t pstride = (size_t)nx * ny;
+  const size_t col_main = (size_t)jm * nx + im, col_yh = (size_t)jh * nx + im, col_xh = (size_t)jxh * nx + ixh;
+
+  auto load_cell = [&](size_t id, double* q_, double* w_) {
+#pragma unroll
+    for (int v = 0; v < NC; ++v) q_[v] = __ldg(qin.r[v] + id);
+#pragma unroll
+    for (int v = 0; v < NH; ++v) w_[v] = __ldg(win.r[v] + id);
+  };
+  auto load_mx = [&](size_t id, double* B, double* E, double& psi, double& phi) {
+#pragma unroll
+    for (int d = 0; d < 3; ++d) { B[d] = __ldg(qin.r[FS::IB + d] + id); E[d] = __ldg(qin.r[FS::IE + d] + id); }
+    psi = __ldg(qin.r[FS::IPSI] + id); phi = __ldg(qin.r[FS::IPHI] + id);
+  };
+  auto prefetch_cell = [&](size_t id) {
+#pragma unroll
+    for (int v = 0; v < NC; ++v) prefetch_l2(qin.r[v] + id);
+#pragma unroll
+    for (int v = 0; v < NH; ++v) prefetch_l2(win.r[v] + id);
+  };
+
+  const int k0 = HAS_Z ? blockIdx.z * seg_len : 0;
+  const int k1 = HAS_Z ? min(nz, k0 + seg_len) : 1;
+  // z carry: pending left-biased reconstructions of the newest face, G of the previous face (own rows only)
+  double pend[NHV], Gprev[NM];                      // H uses pend[0..5], Gprev[0..5]; M uses pend[0..3], Gprev[0..7]
+#pragma unroll
+  for (int v = 0; v < NHV; ++v) pend[v] = 0.0;
+#pragma unroll
+  for (int v = 0; v < NM; ++v) Gprev[v] = 0.0;
+  int s_old = 0, s_new = 2 * NHV * FF_MAIN;
+
+  const int cbeg = HAS_Z ? k0 - 2 : 2, cend = HAS_Z ? k1 + 1 : 2;
+#pragma unroll 1
+  for (int c = cbeg; c <= cend; ++c) {
+    const int k = HAS_Z ? c - 2 : 0;
+    const bool do_xy = !HAS_Z || c >= k0 + 2;
+    const size_t pk = (size_t)k * pstride;
+    double Lacc[NM];                                 // H: 6 rows (D, S, tau, rho_charge); M: 8 rows (B, E, psi, phi)
+#pragma unroll
+    for (int v = 0; v < NM; ++v) Lacc[v] = 0.0;
+
+    if (roleH) {
+      // ======================================= role H =======================================
+      if (do_xy) {
+        if (HAS_Z && c < cend) prefetch_cell((size_t)bc_map(c + 1, nz, bcz) * pstride + col_main);
+        {
+          double q_[NC], w_[NH], fh[NHV];
+          Com<0> cm;
+          load_cell(pk + col_main, q_, w_);
+          cell_common(q_, w_, P, cm);
+          cell_hflux<0>(q_, w_, cm, P, fh);
+#pragma unroll
+          for (int h = 0; h < NHV; ++h) {
+            gX[(h * TY + ty) * XW + lane + 2] = fh[h] + q_[FS::hv(h)];
+            gX[((NHV + h) * TY + ty) * XW + lane + 2] = fh[h] - q_[FS::hv(h)];
+          }
+          cell_hflux<1>(q_, w_, cm, P, fh);
+#pragma unroll
+          for (int h = 0; h < NHV; ++h) {
+            gY[(h * YR + ty + 2) * TX + lane] = fh[h] + q_[FS::hv(h)];
+            gY[((NHV + h) * YR + ty + 2) * TX + lane] = fh[h] - q_[FS::hv(h)];
+          }
+        }
+        hm_barrier();
+        {
+          double o[2 * NHV];
+          face_recon_range<0, 2 * NHV, RMHD_HM_GH>(gX + ty * XW + lane, FSX, 1, o);
+#pragma unroll
+          for (int h = 0; h < NHV; ++h) {
+            const double G = o[h] + o[NHV + h];
+            const double Gr = __shfl_down_sync(0xffffffffu, G, 1);
+            Lacc[h] = (lane < 31 ? G - Gr : G) * hidx;
+          }
+          face_recon_range<0, 2 * NHV, RMHD_HM_GH>(gY + ty * TX + lane, FSY, TX, o);
+#pragma unroll
+          for (int h = 0; h < NHV; ++h) {
+            const double G = o[h] + o[NHV + h];
+            fY[(FS::hv(h) * (TY + 1) + ty) * TX + lane] = G;
+            Lacc[h] = fma(G, hidy, Lacc[h]);
+          }
+          if (wrp == 0) {                            // 5th row of y-faces
+            face_recon_range<0, 2 * NHV, RMHD_HM_GH>(gY + TY * TX + lane, FSY, TX, o);
+#pragma unroll
+            for (int h = 0; h < NHV; ++h) fY[(FS::hv(h) * (TY + 1) + TY) * TX + lane] = o[h] + o[NHV + h];
+          } else if (wrp == 1 && lane < TY) {        // 33rd x-face of row `lane`
+            face_recon_range<0, 2 * NHV, RMHD_HM_GH>(gX + lane * XW + TX, FSX, 1, o);
+#pragma unroll
+            for (int h = 0; h < NHV; ++h) fX[FS::hv(h) * TY + lane] = o[h] + o[NHV + h];
+          }
+        }
+        hm_barrier();
+#pragma unroll
+        for (int h = 0; h < NHV; ++h) Lacc[h] = fma(-fY[(FS::hv(h) * (TY + 1) + ty + 1) * TX + lane], hidy, Lacc[h]);
+        if (lane == 31) {
+#pragma unroll
+          for (int h = 0; h < NHV; ++h) Lacc[h] = fma(-fX[FS::hv(h) * TY + ty], hidx, Lacc[h]);
+        }
+      }
+      if (HAS_Z) {
+        double u0[2 * NHV];
+        {
+          double q_[NC], w_[NH], fh[NHV];
+          Com<0> cm;
+          load_cell((size_t)bc_map(c, nz, bcz) * pstride + col_main, q_, w_);
+          cell_common(q_, w_, P, cm);
+          cell_hflux<2>(q_, w_, cm, P, fh);
+#pragma unroll
+          for (int h = 0; h < NHV; ++h) { u0[h] = fh[h] + q_[FS::hv(h)]; u0[NHV + h] = fh[h] - q_[FS::hv(h)]; }
+        }
+        if (c >= k0) {
+          double o[2 * NHV];
+#pragma unroll
+          for (int f0 = 0; f0 < 2 * NHV; f0 += RMHD_HM_GH) {
+            constexpr int G = RMHD_HM_GH;
+            double a[G], b[G], cc[G];
+#pragma unroll
+            for (int g = 0; g < G; ++g) {
+              const int f = f0 + g;
+              const double u2 = ring[s_old + f * FF_MAIN];
+              b[g] = ring[s_new + f * FF_MAIN];
+              if (f < NHV) { a[g] = u2; cc[g] = u0[f]; } else { a[g] = u0[f]; cc[g] = u2; }
+            }
+            weno3_batch<G, true>(a, b, cc, o + f0);
+          }
+#pragma unroll
+          for (int h = 0; h < NHV; ++h) {
+            const double G = pend[h] + o[NHV + h];   // face c-3/2: last step's "+" and this step's "-"
+            pend[h] = o[h];
+            if (do_xy) Lacc[h] = fma(Gprev[h] - G, hidz, Lacc[h]);
+            Gprev[h] = G;
+          }
+        }
+#pragma unroll
+        for (int f = 0; f < 2 * NHV; ++f) ring[s_old + f * FF_MAIN] = u0[f];
+        { const int t = s_old; s_old = s_new; s_new = t; }
+      }
+      if (do_xy && inside) {
+        const size_t id = pk + (size_t)j * nx + i;
+#pragma unroll
+        for (int h = 0; h < NHV; ++h) L[(size_t)FS::hv(h) * N + id] = Lacc[h];
+      }
+    } else {
+      // ======================================= role M =======================================
+      if (do_xy) {
+        if (HAS_Z && c < cend) {
+          const size_t pn = (size_t)(k + 1) * pstride;
+          prefetch_cell(pn + col_yh);
+          if (wrp == 2 * TY - 1 && lane < 16) prefetch_cell(pn + col_xh);
+        }
+        {
+          double B[3], E[3], psi, phi, m[NM];
+          load_mx(pk + col_main, B, E, psi, phi);
+          mx_fields<0>(B, E, psi, phi, m);
+#pragma unroll
+          for (int f = 0; f < NM; ++f) gX[((2 * NHV + f) * TY + ty) * XW + lane + 2] = m[f];
+          mx_fields<1>(B, E, psi, phi, m);
+#pragma unroll
+          for (int f = 0; f < NM; ++f) gY[((2 * NHV + f) * YR + ty + 2) * TX + lane] = m[f];
+        }
+        {
+          double q_[NC], w_[NH], g[NF];
+          Com<0> cm;
+          load_cell(pk + col_yh, q_, w_);
+          cell_common(q_, w_, P, cm);
+          cell_fields<0, 1>(q_, w_, cm, P, g);
+#pragma unroll
+          for (int f = 0; f < NF; ++f) gY[(f * YR + hrow) * TX + lane] = g[f];
+          if (wrp == 2 * TY - 1 && lane < 16) {
+            load_cell(pk + col_xh, q_, w_);
+            cell_common(q_, w_, P, cm);
+            cell_fields<0, 0>(q_, w_, cm, P, g);
+#pragma unroll
+            for (int f = 0; f < NF; ++f) gX[(f * TY + xh_row) * XW + xh_col] = g[f];
+          }
+        }
+        hm_barrier();
+        {
+          double o[NM], G[NM];
+          face_recon_range<2 * NHV, NM, NM>(gX + ty * XW + lane, FSX, 1, o);
+          assemble_M<0>(o, G);
+#pragma unroll
+          for (int v = 0; v < NM; ++v) {
+            const double Gr = __shfl_down_sync(0xffffffffu, G[v], 1);
+            Lacc[v] = (lane < 31 ? G[v] - Gr : G[v]) * hidx;
+          }
+          face_recon_range<2 * NHV, NM, NM>(gY + ty * TX + lane, FSY, TX, o);
+          assemble_M<1>(o, G);
+#pragma unroll
+          for (int v = 0; v < NM; ++v) { fY[(hm_mrow(v) * (TY + 1) + ty) * TX + lane] = G[v]; Lacc[v] = fma(G[v], hidy, Lacc[v]); }
+          if (wrp == TY) {
+            face_recon_range<2 * NHV, NM, NM>(gY + TY * TX + lane, FSY, TX, o);
+            assemble_M<1>(o, G);
+#pragma unroll
+            for (int v = 0; v < NM; ++v) fY[(hm_mrow(v) * (TY + 1) + TY) * TX + lane] = G[v];
+          } else if (wrp == TY + 1 && lane < TY) {
+            face_recon_range<2 * NHV, NM, NM>(gX + lane * XW + TX, FSX, 1, o);
+            assemble_M<0>(o, G);
+#pragma unroll
+            for (int v = 0; v < NM; ++v) fX[hm_mrow(v) * TY + lane] = G[v];
+          }
+        }
+        hm_barrier();
+#pragma unroll
+        for (int v = 0; v < NM; ++v) Lacc[v] = fma(-fY[(hm_mrow(v) * (TY + 1) + ty + 1) * TX + lane], hidy, Lacc[v]);
+        if (lane == 31) {
+#pragma unroll
+          for (int v = 0; v < NM; ++v) Lacc[v] = fma(-fX[hm_mrow(v) * TY + ty], hidx, Lacc[v]);
+        }
+      }
+      if (HAS_Z) {
+        double u0[NM], u1[NM], u2[NM];
+        {
+          double B[3], E[3], psi, phi;
+          load_mx((size_t)bc_map(c, nz, bcz) * pstride + col_main, B, E, psi, phi);
+          mx_fields<2>(B, E, psi, phi, u0);
+          load_mx((size_t)bc_map(c - 1, nz, bcz) * pstride + col_main, B, E, psi, phi);
+          mx_fields<2>(B, E, psi, phi, u1);
+          load_mx((size_t)bc_map(c - 2, nz, bcz) * pstride + col_main, B, E, psi, phi);
+          mx_fields<2>(B, E, psi, phi, u2);
+        }
+        if (c >= k0) {
+          double a[NM], cc[NM], o[NM], oo[NM], G[NM];
+#pragma unroll
+          for (int g = 0; g < NM; ++g) { if (g < 4) { a[g] = u2[g]; cc[g] = u0[g]; } else { a[g] = u0[g]; cc[g] = u2[g]; } }
+          weno3_batch<NM, true>(a, u1, cc, o);
+#pragma unroll
+          for (int g = 0; g < 4; ++g) { oo[g] = pend[g]; pend[g] = o[g]; oo[4 + g] = o[4 + g]; }
+          assemble_M<2>(oo, G);
+#pragma unroll
+          for (int v = 0; v < NM; ++v) { if (do_xy) Lacc[v] = fma(Gprev[v] - G[v], hidz, Lacc[v]); Gprev[v] = G[v]; }
+        }
+      }
+      if (do_xy && inside) {
+        const size_t id = pk + (size_t)j * nx + i;
+#pragma unroll
+        for (int v = 0; v < NM; ++v) L[(size_t)hm_mrow(v) * N + id] = Lacc[v];
+      }
+    }
+  }
+}
+
+}  // namespace rmhd

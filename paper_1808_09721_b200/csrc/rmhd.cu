@@ -10,6 +10,7 @@
 
 #include "kernels.cuh"
 #include "flux_fused.cuh"
+#include "flux_hm.cuh"
 
 using namespace rmhd;
 
@@ -38,6 +39,7 @@ struct rmhd_ctx {
   Stats* h_stats;  // pinned
   bool profiling;
   bool fused_flux;   // one-pass L(q) over all axes (flux_fused.cuh) when nx, ny > 1; RMHD_FLUX=split forces the per-axis kernels
+  bool one_role;     // RMHD_FLUX=fused1: resistive model through the one-thread-per-column kernel (flux_fused.cuh) instead of flux_hm.cuh
   int sm_count;
   std::vector<EvRec> pending;
   std::vector<cudaEvent_t> ev_pool;
@@ -156,6 +158,7 @@ int launch_flux_fused(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODE
   const size_t smem = FFSmem<MODEL>::bytes(HAS_Z);
   if (!attr_set[c->device & 7]) {
     CK(c, cudaFuncSetAttribute(k_flux_fused<MODEL, HAS_Z>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if constexpr (MODEL == 0) CK(c, cudaFuncSetAttribute(k_flux_hm<HAS_Z>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     attr_set[c->device & 7] = true;
   }
   const int gx = (nx + FF_TX - 1) / FF_TX, gy = (ny + FF_TY - 1) / FF_TY;
@@ -174,8 +177,16 @@ int launch_flux_fused(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODE
   }
   dim3 grid(gx, gy, nseg);
   Timed t(c, KC_FLUX);
-  k_flux_fused<MODEL, HAS_Z><<<grid, FF_THREADS, smem, c->stream>>>(qr, wr, L, c->N, nx, ny, nz, c->p.bc[0], c->p.bc[1], c->p.bc[2],
-                                                                   0.5 / c->dx[0], 0.5 / c->dx[1], 0.5 / c->dx[2], seg_len, c->P);
+  bool two_role = false;
+  if constexpr (MODEL == 0) two_role = !c->one_role;
+  if constexpr (MODEL == 0) {
+    if (two_role)
+      k_flux_hm<HAS_Z><<<grid, HM_THREADS, smem, c->stream>>>(qr, wr, L, c->N, nx, ny, nz, c->p.bc[0], c->p.bc[1], c->p.bc[2],
+                                                            0.5 / c->dx[0], 0.5 / c->dx[1], 0.5 / c->dx[2], seg_len, c->P);
+  }
+  if (!two_role)
+    k_flux_fused<MODEL, HAS_Z><<<grid, FF_THREADS, smem, c->stream>>>(qr, wr, L, c->N, nx, ny, nz, c->p.bc[0], c->p.bc[1], c->p.bc[2],
+                                                                     0.5 / c->dx[0], 0.5 / c->dx[1], 0.5 / c->dx[2], seg_len, c->P);
   CK(c, cudaGetLastError());
   return RMHD_OK;
 }
@@ -278,6 +289,7 @@ int rmhd_create(const rmhd_params* p, rmhd_ctx** out) {
   c->nsteps = 0; c->device = p->device; c->stream = (cudaStream_t)p->stream;
   c->profiling = false;
   { const char* e = getenv("RMHD_FLUX"); c->fused_flux = !(e && strcmp(e, "split") == 0); }
+  { const char* e = getenv("RMHD_FLUX"); c->one_role = e && strcmp(e, "fused1") == 0; }
   c->sm_count = 148;
   for (int i = 0; i < KC_N; ++i) { c->ms[i] = 0.0; c->launches[i] = 0; }
   c->q = c->w = c->qs = c->L1 = c->L2 = c->Ps1 = c->Ps2 = nullptr; c->d_stats = nullptr; c->h_stats = nullptr;
