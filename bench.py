@@ -243,12 +243,13 @@ def run_ours(args):
     value = world * ncell * args.steps / (ms_total * 1e-3)
 
     # ---- roofline of the dominant kernel class -------------------------------------------------
-    naxes = sum(1 for n in (nx, ny, nz) if n > 1)
     dom = max(("stage1", "stage2", "flux", "combine_c2p"), key=lambda k: kt[k]["ms"])
     avg_ms = kt[dom]["ms"] / max(kt[dom]["launches"], 1)
     shares = {k: round(v["ms"] / max(sum(x["ms"] for x in kt.values()), 1e-30), 4) for k, v in kt.items()}
     alg_bytes = {  # SURVEY.md 8(d) table, doubles per cell per launch x 8 B (resistive)
-        "stage1": 29 * 8 * ncell, "stage2": 57 * 8 * ncell, "flux": 33 * 8 * ncell / max(naxes, 1),
+        "stage1": 29 * 8 * ncell, "stage2": 57 * 8 * ncell,
+        # one L(q) evaluation = 33 doubles per cell; the fused kernel does it in 1 launch, the split path in naxes
+        "flux": 33 * 8 * ncell * 2 * args.steps / max(kt["flux"]["launches"], 1),
         "combine_c2p": 76 * 8 * ncell,   # 76 incl. the fused F2 reads; the un-fused kernel's own minimum is 62
     }
     if dom in ("stage1", "stage2"):
