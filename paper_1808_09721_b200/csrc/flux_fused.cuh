@@ -183,10 +183,37 @@ template <int MODEL> struct FFSmem {
   static constexpr size_t bytes(bool has_z) { return sizeof(double) * (GX + GY + FY + FX + (has_z ? RING : 0)); }
 };
 
-template <int MODEL, bool HAS_Z>
+// a5 fused into the F2 launch (COMB = true): the kernel does not store L2 but finishes eq (11) row by row,
+//   q^{n+1}_v = A_v + hdt L2_v,   A_v = qn_v + hdt L1_v + hdt (Psi1_v + Psi2_v) left by stage 2 in the L2 buffer,
+//   hdt = dt/2 (w = w~ = (1/2, 1/2), Table 2),
+// into the qn rows (F2 reads the stage state qs, never qn), so L2 is neither written nor re-read.
+struct FluxComb { double* q; const double* A; double hdt; };
+// store NR rows (row index by ROW(r)) of one cell: L itself, or the eq-(11) update
+template <bool COMB, int NR, class ROW>
+RMHD_DEV void store_rows(double* __restrict__ L, const FluxComb& cb, size_t N, size_t id, const double* Lacc, ROW row) {
+  if constexpr (!COMB) {
+#pragma unroll
+    for (int r = 0; r < NR; ++r) L[(size_t)row(r) * N + id] = Lacc[r];
+  } else {
+    double x[NR];
+#pragma unroll
+    for (int r = 0; r < NR; ++r) x[r] = __ldg(cb.A + (size_t)row(r) * N + id);
+#pragma unroll
+    for (int r = 0; r < NR; ++r) cb.q[(size_t)row(r) * N + id] = fma(cb.hdt, Lacc[r], x[r]);
+  }
+}
+template <bool COMB, int NR, class ROW>
+RMHD_DEV void prefetch_rows(const FluxComb& cb, size_t N, size_t id, ROW row) {
+  if constexpr (COMB) {
+#pragma unroll
+    for (int r = 0; r < NR; ++r) prefetch_l2(cb.A + (size_t)row(r) * N + id);
+  }
+}
+
+template <int MODEL, bool HAS_Z, bool COMB = false>
 __global__ void __launch_bounds__(FF_THREADS, (MODEL == 0 || !HAS_Z) ? 2 : 1)
 k_flux_fused(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, size_t N, int nx, int ny, int nz, int bcx, int bcy,
-             int bcz, double hidx, double hidy, double hidz, int seg_len, DevPar P) {
+             int bcz, double hidx, double hidy, double hidz, int seg_len, DevPar P, FluxComb cb) {
   using FS = FSet<MODEL>;
   using SM = FFSmem<MODEL>;
   constexpr int NC = Dim<MODEL>::NC, NH = Dim<MODEL>::NH, NF = FS::NF, NHV = FS::NHV;
@@ -240,6 +267,7 @@ k_flux_fused(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, si
     if (do_xy) {
       const size_t pk = (size_t)k * pstride;
       // ---------------- P1: fields of the tile and its halo -> shared memory ------------------------
+      if (inside) prefetch_rows<COMB, NC>(cb, N, pk + (size_t)j * nx + i, [](int r) { return r; });
       if (HAS_Z && c < cend) {                      // L2 prefetch of what the next iteration loads first
         const size_t pn = (size_t)(k + 1) * pstride;
         if (is_main) { prefetch_cell(pn + col_yh); prefetch_cell((size_t)bc_map(c + 1, nz, bcz) * pstride + col_main); }
@@ -367,8 +395,7 @@ k_flux_fused(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, si
     }
     if (do_xy && inside) {
       const size_t id = (size_t)k * pstride + (size_t)j * nx + i;
-#pragma unroll
-      for (int v = 0; v < NC; ++v) L[(size_t)v * N + id] = Lacc[v];
+      store_rows<COMB, NC>(L, cb, N, id, Lacc, [](int r) { return r; });
     }
   }
 }

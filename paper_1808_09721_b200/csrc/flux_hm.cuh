@@ -56,10 +56,10 @@ __host__ __device__ constexpr int hm_mrow(int m) { return m < 6 ? 5 + m : (m == 
 #define RMHD_HM_GH 6     // reconstructions in flight per batch, role H (12 per face)
 #endif
 
-template <bool HAS_Z>
+template <bool HAS_Z, bool COMB = false>
 __global__ void __launch_bounds__(HM_THREADS, 2)
 k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int nx, int ny, int nz, int bcx, int bcy, int bcz,
-          double hidx, double hidy, double hidz, int seg_len, DevPar P) {
+          double hidx, double hidy, double hidz, int seg_len, DevPar P, FluxComb cb) {
   using FS = FSet<0>;
   using SM = FFSmem<0>;
   constexpr int NC = R_NC, NH = R_NH, NF = FS::NF, NHV = FS::NHV, NM = 8;
@@ -127,6 +127,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
       // ======================================= role H =======================================
       if (do_xy) {
         if (HAS_Z && c < cend) prefetch_cell((size_t)bc_map(c + 1, nz, bcz) * pstride + col_main);
+        if (inside) prefetch_rows<COMB, NHV>(cb, N, pk + (size_t)j * nx + i, [](int h) { return FS::hv(h); });
         {
           double q_[NC], w_[NH], fh[NHV];
           Com<0> cm;
@@ -220,12 +221,12 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
       }
       if (do_xy && inside) {
         const size_t id = pk + (size_t)j * nx + i;
-#pragma unroll
-        for (int h = 0; h < NHV; ++h) L[(size_t)FS::hv(h) * N + id] = Lacc[h];
+        store_rows<COMB, NHV>(L, cb, N, id, Lacc, [](int h) { return FS::hv(h); });
       }
     } else {
       // ======================================= role M =======================================
       if (do_xy) {
+        if (inside) prefetch_rows<COMB, NM>(cb, N, pk + (size_t)j * nx + i, [](int m) { return hm_mrow(m); });
         if (HAS_Z && c < cend) {
           const size_t pn = (size_t)(k + 1) * pstride;
           prefetch_cell(pn + col_yh);
@@ -316,8 +317,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
       }
       if (do_xy && inside) {
         const size_t id = pk + (size_t)j * nx + i;
-#pragma unroll
-        for (int v = 0; v < NM; ++v) L[(size_t)hm_mrow(v) * N + id] = Lacc[v];
+        store_rows<COMB, NM>(L, cb, N, id, Lacc, [](int m) { return hm_mrow(m); });
       }
     }
   }

@@ -169,12 +169,16 @@ __global__ void __launch_bounds__(256) k_con2prim(const double* __restrict__ con
 //   STAGE 1: q_ex = qn.                       writes E*, psi*, phi* rows of qs, prims, Psi1
 //   STAGE 2: q_ex = qn + dt L1 + (1-2g) dt Psi1 (fused a5).  writes all rows of qs, prims, Psi2
 // Psi rows stored: -J (3), rhoc - kappa psi*, -kappa phi*.
+// MKA (stage 2 on the fused-flux path): instead of Psi2 the kernel writes the part of eq (11) that is known
+// once stage 2 is solved,  A_v = qn_v + hdt L1_v + hdt (Psi1_v + Psi2_v)  (all NC rows, into the buffer that
+// would have held L2), so that the F2 flux launch finishes the step with q^{n+1}_v = A_v + hdt L2_v
+// (flux_fused.cuh, FluxComb).
 // =======================================================================================
-template <int STAGE>
-__global__ void __launch_bounds__(128) k_stage_resistive(const double* __restrict__ qn, const double* __restrict__ L1,
+template <int STAGE, bool MKA = false>
+__global__ void __launch_bounds__(128, 4) k_stage_resistive(const double* __restrict__ qn, const double* __restrict__ L1,
                                                          const double* __restrict__ Ps1, double* __restrict__ w,
-                                                         double* __restrict__ qs, double* __restrict__ Ps, size_t N, double a,
-                                                         double cL, double cP, DevPar P, Stats* st) {
+                                                         double* __restrict__ qs, double* __restrict__ Ps, double* __restrict__ A,
+                                                         size_t N, double a, double cL, double cP, double hdt, DevPar P, Stats* st) {
   __shared__ int shist[NBINS];
   BlockHist bh; bh.init(shist);
   const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -188,7 +192,11 @@ __global__ void __launch_bounds__(128) k_stage_resistive(const double* __restric
     for (int v = 0; v < R_NC; ++v) qe[v] = qn[(size_t)v * N + c];
     if (STAGE == 2) {
 #pragma unroll
-      for (int v = 0; v < R_NC; ++v) qe[v] += cL * L1[(size_t)v * N + c];
+      for (int v = 0; v < R_NC; ++v) {
+        const double l = L1[(size_t)v * N + c];
+        if (MKA && (v < 8 || v == 11)) A[(size_t)v * N + c] = fma(hdt, l, qe[v]);
+        qe[v] = fma(cL, l, qe[v]);
+      }
       qe[8] += cP * Ps1[0 * N + c]; qe[9] += cP * Ps1[1 * N + c]; qe[10] += cP * Ps1[2 * N + c];
       qe[12] += cP * Ps1[3 * N + c]; qe[13] += cP * Ps1[4 * N + c];
 #pragma unroll
@@ -204,11 +212,23 @@ __global__ void __launch_bounds__(128) k_stage_resistive(const double* __restric
   }
   if (valid) {
     Hyd h; double J[3], psi, phi;
+    double Ap[R_NS];
+    if (MKA) {       // qn, L1, Psi1 of the source rows again (L2 hits) rather than 10 registers held across the Newton loop
+#pragma unroll
+      for (int k = 0; k < R_NS; ++k) {
+        const size_t v = k < 3 ? 8 + k : 9 + k;
+        Ap[k] = fma(hdt, L1[v * N + c] + Ps1[(size_t)k * N + c], qn[v * N + c]);
+      }
+    }
     r_stage_finish(s, P, h, J, psi, phi, qpsi, qphi);
     qs[8 * N + c] = s.Ex; qs[9 * N + c] = s.Ey; qs[10 * N + c] = s.Ez; qs[12 * N + c] = psi; qs[13 * N + c] = phi;
     w[c] = h.rho; w[N + c] = h.vx; w[2 * N + c] = h.vy; w[3 * N + c] = h.vz; w[4 * N + c] = h.p;
-    Ps[c] = -J[0]; Ps[N + c] = -J[1]; Ps[2 * N + c] = -J[2];
-    Ps[3 * N + c] = s.rhoc - P.kappa * psi; Ps[4 * N + c] = -P.kappa * phi;
+    const double ps[R_NS] = {-J[0], -J[1], -J[2], s.rhoc - P.kappa * psi, -P.kappa * phi};
+#pragma unroll
+    for (int k = 0; k < R_NS; ++k) {
+      if (MKA) A[(size_t)(k < 3 ? 8 + k : 9 + k) * N + c] = fma(hdt, ps[k], Ap[k]);
+      else Ps[(size_t)k * N + c] = ps[k];
+    }
     bh.add(s.iters);
     if (s.status != 1 || !(h.p > 0.0) || !(h.rho > 0.0)) record_fail(st, (long long)c);
   }
@@ -256,11 +276,11 @@ __global__ void __launch_bounds__(128) k_stage_batch_resistive(const double* __r
 // a1: implicit stage, two-fluid (same launch shape and warp-voted loop as the resistive one).
 // Source rows (Psi storage order): Sbar(3), taubar, E(3), psi, phi  = cons rows 6..9, 13..17.
 // =======================================================================================
-template <int STAGE>
+template <int STAGE, bool MKA = false>
 __global__ void __launch_bounds__(128) k_stage_two_fluid(const double* __restrict__ qn, const double* __restrict__ L1,
                                                          const double* __restrict__ Ps1, double* __restrict__ w,
-                                                         double* __restrict__ qs, double* __restrict__ Ps, size_t N, double a,
-                                                         double cL, double cP, DevPar P, Stats* st) {
+                                                         double* __restrict__ qs, double* __restrict__ Ps, double* __restrict__ A,
+                                                         size_t N, double a, double cL, double cP, double hdt, DevPar P, Stats* st) {
   __shared__ int shist[NBINS];
   BlockHist bh; bh.init(shist);
   const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -274,7 +294,11 @@ __global__ void __launch_bounds__(128) k_stage_two_fluid(const double* __restric
     for (int v = 0; v < T_NC; ++v) qe[v] = qn[(size_t)v * N + c];
     if (STAGE == 2) {
 #pragma unroll
-      for (int v = 0; v < T_NC; ++v) qe[v] += cL * L1[(size_t)v * N + c];
+      for (int v = 0; v < T_NC; ++v) {
+        const double l = L1[(size_t)v * N + c];
+        if (MKA && (v < 6 || (v >= 10 && v < 13))) A[(size_t)v * N + c] = fma(hdt, l, qe[v]);
+        qe[v] = fma(cL, l, qe[v]);
+      }
 #pragma unroll
       for (int k = 0; k < T_NS; ++k) qe[k < 4 ? 6 + k : 9 + k] += cP * Ps1[(size_t)k * N + c];
 #pragma unroll
@@ -299,7 +323,12 @@ __global__ void __launch_bounds__(128) k_stage_two_fluid(const double* __restric
 #pragma unroll
     for (int v = 0; v < T_NH; ++v) w[(size_t)v * N + c] = wl[v];
 #pragma unroll
-    for (int k = 0; k < T_NS; ++k) Ps[(size_t)k * N + c] = src[k];
+    for (int k = 0; k < T_NS; ++k) {
+      if (MKA) {
+        const size_t v = k < 4 ? 6 + k : 9 + k;
+        A[v * N + c] = fma(hdt, src[k], fma(hdt, L1[v * N + c] + Ps1[(size_t)k * N + c], qn[v * N + c]));
+      } else Ps[(size_t)k * N + c] = src[k];
+    }
     bh.add(s.iters);
     if (s.status != 1 || !(wl[0] > 0.0) || !(wl[4] > 0.0) || !(wl[5] > 0.0) || !(wl[9] > 0.0)) record_fail(st, (long long)c);
   }

@@ -39,6 +39,7 @@ struct rmhd_ctx {
   Stats* h_stats;  // pinned
   bool profiling;
   bool fused_flux;   // one-pass L(q) over all axes (flux_fused.cuh) when nx, ny > 1; RMHD_FLUX=split forces the per-axis kernels
+  bool fuse_combine; // eq (11) in the epilogue of the F2 flux launch (fused path only); RMHD_COMBINE=split keeps k_final
   bool one_role;     // RMHD_FLUX=fused1: resistive model through the one-thread-per-column kernel (flux_fused.cuh) instead of flux_hm.cuh
   int sm_count;
   std::vector<EvRec> pending;
@@ -151,14 +152,14 @@ int launch_flux_axis(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODEL
 }
 
 // all present axes in one pass (flux_fused.cuh); needs nx > 1 and ny > 1
-template <int MODEL, bool HAS_Z>
-int launch_flux_fused(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODEL>& wr, double* L) {
+template <int MODEL, bool HAS_Z, bool COMB>
+int launch_flux_fused(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODEL>& wr, double* L, const FluxComb& cb) {
   static bool attr_set[8] = {false, false, false, false, false, false, false, false};
   const int nx = c->n[0], ny = c->n[1], nz = c->n[2];
   const size_t smem = FFSmem<MODEL>::bytes(HAS_Z);
   if (!attr_set[c->device & 7]) {
-    CK(c, cudaFuncSetAttribute(k_flux_fused<MODEL, HAS_Z>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    if constexpr (MODEL == 0) CK(c, cudaFuncSetAttribute(k_flux_hm<HAS_Z>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CK(c, cudaFuncSetAttribute(k_flux_fused<MODEL, HAS_Z, COMB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if constexpr (MODEL == 0) CK(c, cudaFuncSetAttribute(k_flux_hm<HAS_Z, COMB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     attr_set[c->device & 7] = true;
   }
   const int gx = (nx + FF_TX - 1) / FF_TX, gy = (ny + FF_TY - 1) / FF_TY;
@@ -181,26 +182,34 @@ int launch_flux_fused(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODE
   if constexpr (MODEL == 0) two_role = !c->one_role;
   if constexpr (MODEL == 0) {
     if (two_role)
-      k_flux_hm<HAS_Z><<<grid, HM_THREADS, smem, c->stream>>>(qr, wr, L, c->N, nx, ny, nz, c->p.bc[0], c->p.bc[1], c->p.bc[2],
-                                                            0.5 / c->dx[0], 0.5 / c->dx[1], 0.5 / c->dx[2], seg_len, c->P);
+      k_flux_hm<HAS_Z, COMB><<<grid, HM_THREADS, smem, c->stream>>>(qr, wr, L, c->N, nx, ny, nz, c->p.bc[0], c->p.bc[1], c->p.bc[2],
+                                                                  0.5 / c->dx[0], 0.5 / c->dx[1], 0.5 / c->dx[2], seg_len, c->P, cb);
   }
   if (!two_role)
-    k_flux_fused<MODEL, HAS_Z><<<grid, FF_THREADS, smem, c->stream>>>(qr, wr, L, c->N, nx, ny, nz, c->p.bc[0], c->p.bc[1], c->p.bc[2],
-                                                                     0.5 / c->dx[0], 0.5 / c->dx[1], 0.5 / c->dx[2], seg_len, c->P);
+    k_flux_fused<MODEL, HAS_Z, COMB><<<grid, FF_THREADS, smem, c->stream>>>(qr, wr, L, c->N, nx, ny, nz, c->p.bc[0], c->p.bc[1], c->p.bc[2],
+                                                                           0.5 / c->dx[0], 0.5 / c->dx[1], 0.5 / c->dx[2], seg_len, c->P, cb);
   CK(c, cudaGetLastError());
   return RMHD_OK;
 }
 
 // L(q) with the conserved rows taken from `qa` except the rows listed in src rows, which come
 // from `qb` when mix != 0 (stage 1 only rewrites the rows that have a source).
+inline bool uses_fused_flux(const rmhd_ctx* c) { return c->fused_flux && c->n[0] > 1 && c->n[1] > 1; }
+
+// `cb` (fused path only): store the eq-(11) update of q instead of L (a5 fused into F2)
 template <int MODEL>
-int launch_flux(rmhd_ctx* c, const double* qa, const double* qb, bool mix, const double* w, double* L) {
+int launch_flux(rmhd_ctx* c, const double* qa, const double* qb, bool mix, const double* w, double* L, const FluxComb* cb = nullptr) {
   constexpr int NC = Dim<MODEL>::NC, NH = Dim<MODEL>::NH, NS = Dim<MODEL>::NS;
   ConsRows<MODEL> qr; HydRows<MODEL> wr;
   for (int v = 0; v < NC; ++v) qr.r[v] = qa + (size_t)v * c->N;
   if (mix) for (int k = 0; k < NS; ++k) { int v = MODEL == 0 ? (k < 3 ? 8 + k : 9 + k) : (k < 4 ? 6 + k : 9 + k); qr.r[v] = qb + (size_t)v * c->N; }
   for (int v = 0; v < NH; ++v) wr.r[v] = w + (size_t)v * c->N;
-  if (c->fused_flux && c->n[0] > 1 && c->n[1] > 1) return c->n[2] > 1 ? launch_flux_fused<MODEL, true>(c, qr, wr, L) : launch_flux_fused<MODEL, false>(c, qr, wr, L);
+  if (uses_fused_flux(c)) {
+    const FluxComb none = {nullptr, nullptr, 0.0};
+    if (cb) return c->n[2] > 1 ? launch_flux_fused<MODEL, true, true>(c, qr, wr, L, *cb) : launch_flux_fused<MODEL, false, true>(c, qr, wr, L, *cb);
+    return c->n[2] > 1 ? launch_flux_fused<MODEL, true, false>(c, qr, wr, L, none) : launch_flux_fused<MODEL, false, false>(c, qr, wr, L, none);
+  }
+  if (cb) { c->err = "internal: combine epilogue needs the fused flux kernel"; return RMHD_ERR_BAD_PARAM; }
   int acc = 0, rc;
   if (c->n[0] > 1) { if ((rc = launch_flux_axis<MODEL, 0>(c, qr, wr, L, acc))) return rc; acc = 1; }
   if (c->n[1] > 1) { if ((rc = launch_flux_axis<MODEL, 1>(c, qr, wr, L, acc))) return rc; acc = 1; }
@@ -217,16 +226,31 @@ int step_once(rmhd_ctx* c) {
   int rc;
   {
     Timed t(c, KC_STAGE1);
-    if (MODEL == 0) k_stage_resistive<1><<<nb, 128, 0, c->stream>>>(c->q, nullptr, nullptr, c->w, c->qs, c->Ps1, c->N, g * dt, 0.0, 0.0, c->P, c->d_stats);
-    else k_stage_two_fluid<1><<<nb, 128, 0, c->stream>>>(c->q, nullptr, nullptr, c->w, c->qs, c->Ps1, c->N, g * dt, 0.0, 0.0, c->P, c->d_stats);
+    if (MODEL == 0) k_stage_resistive<1><<<nb, 128, 0, c->stream>>>(c->q, nullptr, nullptr, c->w, c->qs, c->Ps1, nullptr, c->N, g * dt, 0.0, 0.0, 0.0, c->P, c->d_stats);
+    else k_stage_two_fluid<1><<<nb, 128, 0, c->stream>>>(c->q, nullptr, nullptr, c->w, c->qs, c->Ps1, nullptr, c->N, g * dt, 0.0, 0.0, 0.0, c->P, c->d_stats);
     CK(c, cudaGetLastError());
   }
   if ((rc = launch_flux<MODEL>(c, c->q, c->qs, true, c->w, c->L1))) return rc;
+  const bool fuse_c = uses_fused_flux(c) && c->fuse_combine;
   {
     Timed t(c, KC_STAGE2);
-    if (MODEL == 0) k_stage_resistive<2><<<nb, 128, 0, c->stream>>>(c->q, c->L1, c->Ps1, c->w, c->qs, c->Ps2, c->N, g * dt, dt, (1.0 - 2.0 * g) * dt, c->P, c->d_stats);
-    else k_stage_two_fluid<2><<<nb, 128, 0, c->stream>>>(c->q, c->L1, c->Ps1, c->w, c->qs, c->Ps2, c->N, g * dt, dt, (1.0 - 2.0 * g) * dt, c->P, c->d_stats);
+    if (fuse_c) {   // stage 2 leaves A = qn + dt/2 L1 + dt/2 (Psi1 + Psi2) in the L2 buffer
+      if (MODEL == 0) k_stage_resistive<2, true><<<nb, 128, 0, c->stream>>>(c->q, c->L1, c->Ps1, c->w, c->qs, c->Ps2, c->L2, c->N, g * dt, dt, (1.0 - 2.0 * g) * dt, 0.5 * dt, c->P, c->d_stats);
+      else k_stage_two_fluid<2, true><<<nb, 128, 0, c->stream>>>(c->q, c->L1, c->Ps1, c->w, c->qs, c->Ps2, c->L2, c->N, g * dt, dt, (1.0 - 2.0 * g) * dt, 0.5 * dt, c->P, c->d_stats);
+    } else {
+      if (MODEL == 0) k_stage_resistive<2><<<nb, 128, 0, c->stream>>>(c->q, c->L1, c->Ps1, c->w, c->qs, c->Ps2, nullptr, c->N, g * dt, dt, (1.0 - 2.0 * g) * dt, 0.0, c->P, c->d_stats);
+      else k_stage_two_fluid<2><<<nb, 128, 0, c->stream>>>(c->q, c->L1, c->Ps1, c->w, c->qs, c->Ps2, nullptr, c->N, g * dt, dt, (1.0 - 2.0 * g) * dt, 0.0, c->P, c->d_stats);
+    }
     CK(c, cudaGetLastError());
+  }
+  if (fuse_c) {
+    // F2 + C in one launch (q^{n+1} = A + dt/2 L2 row by row in the flux kernel's epilogue), then P: con2prim of q^{n+1}
+    const FluxComb cb = {c->q, c->L2, 0.5 * dt};
+    if ((rc = launch_flux<MODEL>(c, c->qs, nullptr, false, c->w, c->L2, &cb))) return rc;
+    Timed t(c, KC_FINAL);
+    k_con2prim<MODEL><<<blocks_for(c->N, 256), 256, 0, c->stream>>>(c->q, c->w, c->N, c->w, c->N, nullptr, nullptr, nullptr, c->N, c->P, c->d_stats);
+    CK(c, cudaGetLastError());
+    return RMHD_OK;
   }
   if ((rc = launch_flux<MODEL>(c, c->qs, nullptr, false, c->w, c->L2))) return rc;
   {
@@ -290,6 +314,7 @@ int rmhd_create(const rmhd_params* p, rmhd_ctx** out) {
   c->profiling = false;
   { const char* e = getenv("RMHD_FLUX"); c->fused_flux = !(e && strcmp(e, "split") == 0); }
   { const char* e = getenv("RMHD_FLUX"); c->one_role = e && strcmp(e, "fused1") == 0; }
+  { const char* e = getenv("RMHD_COMBINE"); c->fuse_combine = !(e && strcmp(e, "split") == 0); }
   c->sm_count = 148;
   for (int i = 0; i < KC_N; ++i) { c->ms[i] = 0.0; c->launches[i] = 0; }
   c->q = c->w = c->qs = c->L1 = c->L2 = c->Ps1 = c->Ps2 = nullptr; c->d_stats = nullptr; c->h_stats = nullptr;
