@@ -147,30 +147,25 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
           }
         }
         hm_barrier();
-        {
+        // left x-face (t = 0) and bottom y-face (t = 1) of the own cell: ONE copy of the reconstruction code
+#pragma unroll 1
+        for (int t = 0; t < 2; ++t) {
           double o[2 * NHV];
-          face_recon_range<0, 2 * NHV, RMHD_HM_GH>(gX + ty * XW + lane, FSX, 1, o);
+          face_recon_range<0, 2 * NHV, RMHD_HM_GH>(t ? gY + ty * TX + lane : gX + ty * XW + lane, t ? FSY : FSX, t ? TX : 1, o);
+          if (t == 0) {
 #pragma unroll
-          for (int h = 0; h < NHV; ++h) {
-            const double G = o[h] + o[NHV + h];
-            const double Gr = __shfl_down_sync(0xffffffffu, G, 1);
-            Lacc[h] = (lane < 31 ? G - Gr : G) * hidx;
-          }
-          face_recon_range<0, 2 * NHV, RMHD_HM_GH>(gY + ty * TX + lane, FSY, TX, o);
+            for (int h = 0; h < NHV; ++h) {
+              const double G = o[h] + o[NHV + h];
+              const double Gr = __shfl_down_sync(0xffffffffu, G, 1);
+              Lacc[h] = (lane < 31 ? G - Gr : G) * hidx;
+            }
+          } else {
 #pragma unroll
-          for (int h = 0; h < NHV; ++h) {
-            const double G = o[h] + o[NHV + h];
-            fY[(FS::hv(h) * (TY + 1) + ty) * TX + lane] = G;
-            Lacc[h] = fma(G, hidy, Lacc[h]);
-          }
-          if (wrp == 0) {                            // 5th row of y-faces
-            face_recon_range<0, 2 * NHV, RMHD_HM_GH>(gY + TY * TX + lane, FSY, TX, o);
-#pragma unroll
-            for (int h = 0; h < NHV; ++h) fY[(FS::hv(h) * (TY + 1) + TY) * TX + lane] = o[h] + o[NHV + h];
-          } else if (wrp == 1 && lane < TY) {        // 33rd x-face of row `lane`
-            face_recon_range<0, 2 * NHV, RMHD_HM_GH>(gX + lane * XW + TX, FSX, 1, o);
-#pragma unroll
-            for (int h = 0; h < NHV; ++h) fX[FS::hv(h) * TY + lane] = o[h] + o[NHV + h];
+            for (int h = 0; h < NHV; ++h) {
+              const double G = o[h] + o[NHV + h];
+              fY[(FS::hv(h) * (TY + 1) + ty) * TX + lane] = G;
+              Lacc[h] = fma(G, hidy, Lacc[h]);
+            }
           }
         }
         hm_barrier();
@@ -225,6 +220,8 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
       }
     } else {
       // ======================================= role M =======================================
+      // z first: it loads B, E, psi, phi of planes c-2, c-1, c; plane c-2 IS plane k, so the x/y fields of the own
+      // cell are built from the same registers (no second load)
       if (do_xy) {
         if (inside) prefetch_rows<COMB, NM>(cb, N, pk + (size_t)j * nx + i, [](int m) { return hm_mrow(m); });
         if (HAS_Z && c < cend) {
@@ -232,16 +229,42 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
           prefetch_cell(pn + col_yh);
           if (wrp == 2 * TY - 1 && lane < 16) prefetch_cell(pn + col_xh);
         }
+      }
+      {
+        double u0[NM], u1[NM], u2[NM];
         {
-          double B[3], E[3], psi, phi, m[NM];
-          load_mx(pk + col_main, B, E, psi, phi);
-          mx_fields<0>(B, E, psi, phi, m);
+          double B[3], E[3], psi, phi;
+          load_mx((HAS_Z ? (size_t)bc_map(c - 2, nz, bcz) * pstride : pk) + col_main, B, E, psi, phi);
+          if (do_xy) {
+            double m[NM];
+            mx_fields<0>(B, E, psi, phi, m);
 #pragma unroll
-          for (int f = 0; f < NM; ++f) gX[((2 * NHV + f) * TY + ty) * XW + lane + 2] = m[f];
-          mx_fields<1>(B, E, psi, phi, m);
+            for (int f = 0; f < NM; ++f) gX[((2 * NHV + f) * TY + ty) * XW + lane + 2] = m[f];
+            mx_fields<1>(B, E, psi, phi, m);
 #pragma unroll
-          for (int f = 0; f < NM; ++f) gY[((2 * NHV + f) * YR + ty + 2) * TX + lane] = m[f];
+            for (int f = 0; f < NM; ++f) gY[((2 * NHV + f) * YR + ty + 2) * TX + lane] = m[f];
+          }
+          if (HAS_Z) {
+            mx_fields<2>(B, E, psi, phi, u2);
+            load_mx((size_t)bc_map(c - 1, nz, bcz) * pstride + col_main, B, E, psi, phi);
+            mx_fields<2>(B, E, psi, phi, u1);
+            load_mx((size_t)bc_map(c, nz, bcz) * pstride + col_main, B, E, psi, phi);
+            mx_fields<2>(B, E, psi, phi, u0);
+          }
         }
+        if (HAS_Z && c >= k0) {
+          double a[NM], cc[NM], o[NM], oo[NM], G[NM];
+#pragma unroll
+          for (int g = 0; g < NM; ++g) { if (g < 4) { a[g] = u2[g]; cc[g] = u0[g]; } else { a[g] = u0[g]; cc[g] = u2[g]; } }
+          weno3_batch<NM, true>(a, u1, cc, o);
+#pragma unroll
+          for (int g = 0; g < 4; ++g) { oo[g] = pend[g]; pend[g] = o[g]; oo[4 + g] = o[4 + g]; }
+          assemble_M<2>(oo, G);
+#pragma unroll
+          for (int v = 0; v < NM; ++v) { if (do_xy) Lacc[v] = (Gprev[v] - G[v]) * hidz; Gprev[v] = G[v]; }
+        }
+      }
+      if (do_xy) {
         {
           double q_[NC], w_[NH], g[NF];
           Com<0> cm;
@@ -259,29 +282,43 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
           }
         }
         hm_barrier();
-        {
+        // t = 0: left x-face, t = 1: bottom y-face of the own cell; t = 2 (warps TY, TY+1 only): the 5th row of
+        // y-faces / the 33rd x-face of row `lane` (lanes >= TY reconstruct in-bounds garbage that is not stored)
+        const int ntask = wrp < TY + 2 ? 3 : 2;
+#pragma unroll 1
+        for (int t = 0; t < ntask; ++t) {
+          const bool ydir = t == 1 || (t == 2 && wrp == TY);
+          const double* p = t == 0 ? gX + ty * XW + lane : (t == 1 ? gY + ty * TX + lane : (ydir ? gY + TY * TX + lane : gX + lane * XW + TX));
           double o[NM], G[NM];
-          face_recon_range<2 * NHV, NM, NM>(gX + ty * XW + lane, FSX, 1, o);
-          assemble_M<0>(o, G);
+          face_recon_range<2 * NHV, NM, NM>(p, ydir ? FSY : FSX, ydir ? TX : 1, o);
+          if (ydir) assemble_M<1>(o, G); else assemble_M<0>(o, G);
+          if (t == 0) {
 #pragma unroll
-          for (int v = 0; v < NM; ++v) {
-            const double Gr = __shfl_down_sync(0xffffffffu, G[v], 1);
-            Lacc[v] = (lane < 31 ? G[v] - Gr : G[v]) * hidx;
-          }
-          face_recon_range<2 * NHV, NM, NM>(gY + ty * TX + lane, FSY, TX, o);
-          assemble_M<1>(o, G);
+            for (int v = 0; v < NM; ++v) {
+              const double Gr = __shfl_down_sync(0xffffffffu, G[v], 1);
+              Lacc[v] = fma(lane < 31 ? G[v] - Gr : G[v], hidx, Lacc[v]);
+            }
+          } else if (t == 1) {
 #pragma unroll
-          for (int v = 0; v < NM; ++v) { fY[(hm_mrow(v) * (TY + 1) + ty) * TX + lane] = G[v]; Lacc[v] = fma(G[v], hidy, Lacc[v]); }
-          if (wrp == TY) {
-            face_recon_range<2 * NHV, NM, NM>(gY + TY * TX + lane, FSY, TX, o);
-            assemble_M<1>(o, G);
+            for (int v = 0; v < NM; ++v) { fY[(hm_mrow(v) * (TY + 1) + ty) * TX + lane] = G[v]; Lacc[v] = fma(G[v], hidy, Lacc[v]); }
+          } else if (ydir) {
 #pragma unroll
             for (int v = 0; v < NM; ++v) fY[(hm_mrow(v) * (TY + 1) + TY) * TX + lane] = G[v];
-          } else if (wrp == TY + 1 && lane < TY) {
-            face_recon_range<2 * NHV, NM, NM>(gX + lane * XW + TX, FSX, 1, o);
-            assemble_M<0>(o, G);
+          } else if (lane < TY) {
 #pragma unroll
             for (int v = 0; v < NM; ++v) fX[hm_mrow(v) * TY + lane] = G[v];
+          }
+        }
+        if (wrp >= TY + 2) {       // the same two extra face sets of the hydro rows (12 fields), taken off role H
+          const bool ydir = wrp == TY + 2;
+          double o[2 * NHV];
+          face_recon_range<0, 2 * NHV, RMHD_HM_GH>(ydir ? gY + TY * TX + lane : gX + (lane & (TY - 1)) * XW + TX, ydir ? FSY : FSX, ydir ? TX : 1, o);
+          if (ydir) {
+#pragma unroll
+            for (int h = 0; h < NHV; ++h) fY[(FS::hv(h) * (TY + 1) + TY) * TX + lane] = o[h] + o[NHV + h];
+          } else if (lane < TY) {
+#pragma unroll
+            for (int h = 0; h < NHV; ++h) fX[FS::hv(h) * TY + lane] = o[h] + o[NHV + h];
           }
         }
         hm_barrier();
@@ -291,33 +328,10 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
 #pragma unroll
           for (int v = 0; v < NM; ++v) Lacc[v] = fma(-fX[hm_mrow(v) * TY + ty], hidx, Lacc[v]);
         }
-      }
-      if (HAS_Z) {
-        double u0[NM], u1[NM], u2[NM];
-        {
-          double B[3], E[3], psi, phi;
-          load_mx((size_t)bc_map(c, nz, bcz) * pstride + col_main, B, E, psi, phi);
-          mx_fields<2>(B, E, psi, phi, u0);
-          load_mx((size_t)bc_map(c - 1, nz, bcz) * pstride + col_main, B, E, psi, phi);
-          mx_fields<2>(B, E, psi, phi, u1);
-          load_mx((size_t)bc_map(c - 2, nz, bcz) * pstride + col_main, B, E, psi, phi);
-          mx_fields<2>(B, E, psi, phi, u2);
+        if (inside) {
+          const size_t id = pk + (size_t)j * nx + i;
+          store_rows<COMB, NM>(L, cb, N, id, Lacc, [](int m) { return hm_mrow(m); });
         }
-        if (c >= k0) {
-          double a[NM], cc[NM], o[NM], oo[NM], G[NM];
-#pragma unroll
-          for (int g = 0; g < NM; ++g) { if (g < 4) { a[g] = u2[g]; cc[g] = u0[g]; } else { a[g] = u0[g]; cc[g] = u2[g]; } }
-          weno3_batch<NM, true>(a, u1, cc, o);
-#pragma unroll
-          for (int g = 0; g < 4; ++g) { oo[g] = pend[g]; pend[g] = o[g]; oo[4 + g] = o[4 + g]; }
-          assemble_M<2>(oo, G);
-#pragma unroll
-          for (int v = 0; v < NM; ++v) { if (do_xy) Lacc[v] = fma(Gprev[v] - G[v], hidz, Lacc[v]); Gprev[v] = G[v]; }
-        }
-      }
-      if (do_xy && inside) {
-        const size_t id = pk + (size_t)j * nx + i;
-        store_rows<COMB, NM>(L, cb, N, id, Lacc, [](int m) { return hm_mrow(m); });
       }
     }
   }
