@@ -190,23 +190,23 @@ template <int MODEL> struct FFSmem {
 struct FluxComb { double* q; const double* A; double hdt; };
 // store NR rows (row index by ROW(r)) of one cell: L itself, or the eq-(11) update
 template <bool COMB, int NR, class ROW>
-RMHD_DEV void store_rows(double* __restrict__ L, const FluxComb& cb, size_t N, size_t id, const double* Lacc, ROW row) {
+RMHD_DEV void store_rows(double* __restrict__ L, const FluxComb& cb, size_t N, unsigned id, const double* Lacc, ROW row) {
   if constexpr (!COMB) {
 #pragma unroll
-    for (int r = 0; r < NR; ++r) L[(size_t)row(r) * N + id] = Lacc[r];
+    for (int r = 0; r < NR; ++r) (L + (size_t)row(r) * N)[id] = Lacc[r];
   } else {
     double x[NR];
 #pragma unroll
-    for (int r = 0; r < NR; ++r) x[r] = __ldg(cb.A + (size_t)row(r) * N + id);
+    for (int r = 0; r < NR; ++r) x[r] = __ldg((cb.A + (size_t)row(r) * N) + id);
 #pragma unroll
-    for (int r = 0; r < NR; ++r) cb.q[(size_t)row(r) * N + id] = fma(cb.hdt, Lacc[r], x[r]);
+    for (int r = 0; r < NR; ++r) (cb.q + (size_t)row(r) * N)[id] = fma(cb.hdt, Lacc[r], x[r]);
   }
 }
 template <bool COMB, int NR, class ROW>
-RMHD_DEV void prefetch_rows(const FluxComb& cb, size_t N, size_t id, ROW row) {
+RMHD_DEV void prefetch_rows(const FluxComb& cb, size_t N, unsigned id, ROW row) {
   if constexpr (COMB) {
 #pragma unroll
-    for (int r = 0; r < NR; ++r) prefetch_l2(cb.A + (size_t)row(r) * N + id);
+    for (int r = 0; r < NR; ++r) prefetch_l2((cb.A + (size_t)row(r) * N) + id);
   }
 }
 
@@ -267,7 +267,7 @@ k_flux_fused(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, si
     if (do_xy) {
       const size_t pk = (size_t)k * pstride;
       // ---------------- P1: fields of the tile and its halo -> shared memory ------------------------
-      if (inside) prefetch_rows<COMB, NC>(cb, N, pk + (size_t)j * nx + i, [](int r) { return r; });
+      if (inside) prefetch_rows<COMB, NC>(cb, N, (unsigned)(pk + (size_t)j * nx + i), [](int r) { return r; });
       if (HAS_Z && c < cend) {                      // L2 prefetch of what the next iteration loads first
         const size_t pn = (size_t)(k + 1) * pstride;
         if (is_main) { prefetch_cell(pn + col_yh); prefetch_cell((size_t)bc_map(c + 1, nz, bcz) * pstride + col_main); }
@@ -395,7 +395,7 @@ k_flux_fused(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, si
     }
     if (do_xy && inside) {
       const size_t id = (size_t)k * pstride + (size_t)j * nx + i;
-      store_rows<COMB, NC>(L, cb, N, id, Lacc, [](int r) { return r; });
+      store_rows<COMB, NC>(L, cb, N, (unsigned)id, Lacc, [](int r) { return r; });
     }
   }
 }

@@ -82,21 +82,22 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
   const int jh = bc_map(j0 + hrow - 2, ny, bcy);
   const int xh_row = (lane >> 2) & 3, xh_col = (lane & 3) < 2 ? (lane & 3) : (lane & 3) + 32;
   const int ixh = bc_map(i0 + xh_col - 2, nx, bcx), jxh = bc_map(j0 + xh_row, ny, bcy);
-  const size_t pstride = (size_t)nx * ny;
-  const size_t col_main = (size_t)jm * nx + im, col_yh = (size_t)jh * nx + im, col_xh = (size_t)jxh * nx + ixh;
+  // 32-bit element offsets inside a row (N < 2^31, checked by rmhd_create): one IMAD.WIDE per access
+  const unsigned pstride = (unsigned)nx * ny;
+  const unsigned col_main = (unsigned)jm * nx + im, col_yh = (unsigned)jh * nx + im, col_xh = (unsigned)jxh * nx + ixh;
 
-  auto load_cell = [&](size_t id, double* q_, double* w_) {
+  auto load_cell = [&](unsigned id, double* q_, double* w_) {
 #pragma unroll
     for (int v = 0; v < NC; ++v) q_[v] = __ldg(qin.r[v] + id);
 #pragma unroll
     for (int v = 0; v < NH; ++v) w_[v] = __ldg(win.r[v] + id);
   };
-  auto load_mx = [&](size_t id, double* B, double* E, double& psi, double& phi) {
+  auto load_mx = [&](unsigned id, double* B, double* E, double& psi, double& phi) {
 #pragma unroll
     for (int d = 0; d < 3; ++d) { B[d] = __ldg(qin.r[FS::IB + d] + id); E[d] = __ldg(qin.r[FS::IE + d] + id); }
     psi = __ldg(qin.r[FS::IPSI] + id); phi = __ldg(qin.r[FS::IPHI] + id);
   };
-  auto prefetch_cell = [&](size_t id) {
+  auto prefetch_cell = [&](unsigned id) {
 #pragma unroll
     for (int v = 0; v < NC; ++v) prefetch_l2(qin.r[v] + id);
 #pragma unroll
@@ -118,7 +119,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
   for (int c = cbeg; c <= cend; ++c) {
     const int k = HAS_Z ? c - 2 : 0;
     const bool do_xy = !HAS_Z || c >= k0 + 2;
-    const size_t pk = (size_t)k * pstride;
+    const unsigned pk = (unsigned)k * pstride;
     double Lacc[NM];                                 // H: 6 rows (D, S, tau, rho_charge); M: 8 rows (B, E, psi, phi)
 #pragma unroll
     for (int v = 0; v < NM; ++v) Lacc[v] = 0.0;
@@ -126,8 +127,8 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
     if (roleH) {
       // ======================================= role H =======================================
       if (do_xy) {
-        if (HAS_Z && c < cend) prefetch_cell((size_t)bc_map(c + 1, nz, bcz) * pstride + col_main);
-        if (inside) prefetch_rows<COMB, NHV>(cb, N, pk + (size_t)j * nx + i, [](int h) { return FS::hv(h); });
+        if (HAS_Z && c < cend) prefetch_cell((unsigned)bc_map(c + 1, nz, bcz) * pstride + col_main);
+        if (inside) prefetch_rows<COMB, NHV>(cb, N, pk + (unsigned)j * nx + i, [](int h) { return FS::hv(h); });
         {
           double q_[NC], w_[NH], fh[NHV];
           Com<0> cm;
@@ -181,7 +182,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
         {
           double q_[NC], w_[NH], fh[NHV];
           Com<0> cm;
-          load_cell((size_t)bc_map(c, nz, bcz) * pstride + col_main, q_, w_);
+          load_cell((unsigned)bc_map(c, nz, bcz) * pstride + col_main, q_, w_);
           cell_common(q_, w_, P, cm);
           cell_hflux<2>(q_, w_, cm, P, fh);
 #pragma unroll
@@ -215,7 +216,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
         { const int t = s_old; s_old = s_new; s_new = t; }
       }
       if (do_xy && inside) {
-        const size_t id = pk + (size_t)j * nx + i;
+        const unsigned id = pk + (unsigned)j * nx + i;
         store_rows<COMB, NHV>(L, cb, N, id, Lacc, [](int h) { return FS::hv(h); });
       }
     } else {
@@ -223,9 +224,9 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
       // z first: it loads B, E, psi, phi of planes c-2, c-1, c; plane c-2 IS plane k, so the x/y fields of the own
       // cell are built from the same registers (no second load)
       if (do_xy) {
-        if (inside) prefetch_rows<COMB, NM>(cb, N, pk + (size_t)j * nx + i, [](int m) { return hm_mrow(m); });
+        if (inside) prefetch_rows<COMB, NM>(cb, N, pk + (unsigned)j * nx + i, [](int m) { return hm_mrow(m); });
         if (HAS_Z && c < cend) {
-          const size_t pn = (size_t)(k + 1) * pstride;
+          const unsigned pn = (unsigned)(k + 1) * pstride;
           prefetch_cell(pn + col_yh);
           if (wrp == 2 * TY - 1 && lane < 16) prefetch_cell(pn + col_xh);
         }
@@ -234,7 +235,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
         double u0[NM], u1[NM], u2[NM];
         {
           double B[3], E[3], psi, phi;
-          load_mx((HAS_Z ? (size_t)bc_map(c - 2, nz, bcz) * pstride : pk) + col_main, B, E, psi, phi);
+          load_mx((HAS_Z ? (unsigned)bc_map(c - 2, nz, bcz) * pstride : pk) + col_main, B, E, psi, phi);
           if (do_xy) {
             double m[NM];
             mx_fields<0>(B, E, psi, phi, m);
@@ -246,9 +247,9 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
           }
           if (HAS_Z) {
             mx_fields<2>(B, E, psi, phi, u2);
-            load_mx((size_t)bc_map(c - 1, nz, bcz) * pstride + col_main, B, E, psi, phi);
+            load_mx((unsigned)bc_map(c - 1, nz, bcz) * pstride + col_main, B, E, psi, phi);
             mx_fields<2>(B, E, psi, phi, u1);
-            load_mx((size_t)bc_map(c, nz, bcz) * pstride + col_main, B, E, psi, phi);
+            load_mx((unsigned)bc_map(c, nz, bcz) * pstride + col_main, B, E, psi, phi);
             mx_fields<2>(B, E, psi, phi, u0);
           }
         }
@@ -329,7 +330,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
           for (int v = 0; v < NM; ++v) Lacc[v] = fma(-fX[hm_mrow(v) * TY + ty], hidx, Lacc[v]);
         }
         if (inside) {
-          const size_t id = pk + (size_t)j * nx + i;
+          const unsigned id = pk + (unsigned)j * nx + i;
           store_rows<COMB, NM>(L, cb, N, id, Lacc, [](int m) { return hm_mrow(m); });
         }
       }

@@ -300,6 +300,7 @@ int rmhd_create(const rmhd_params* p, rmhd_ctx** out) {
   c->ns = p->model == 0 ? R_NS : T_NS; c->np = p->model == 0 ? 11 : 16;
   c->n[0] = p->nx; c->n[1] = p->ny; c->n[2] = p->nz;
   c->N = (size_t)p->nx * p->ny * p->nz;
+  if (c->N >= (size_t)1 << 31) { g_create_error = "grid too large: the kernels index a row with 32-bit offsets (N < 2^31)"; delete c; return RMHD_ERR_BAD_PARAM; }
   const double lo[3] = {p->xmin, p->ymin, p->zmin}, hi[3] = {p->xmax, p->ymax, p->zmax};
   double inv = 0.0;
   for (int d = 0; d < 3; ++d) {
