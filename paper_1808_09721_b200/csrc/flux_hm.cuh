@@ -21,6 +21,26 @@ constexpr int HM_THREADS = 2 * FF_MAIN;
 // CTA-wide barrier reached from role-specific code paths (every thread executes the same number of them)
 RMHD_DEV void hm_barrier() { asm volatile("bar.sync 1, %0;" ::"n"(HM_THREADS) : "memory"); }
 
+// split-phase CTA barrier (mbarrier): arrive when the own shared-memory reads/writes of a phase are done, wait
+// only where the others' results are needed; independent work placed in between hides the skew between warps
+RMHD_DEV void mbar_init(unsigned long long* bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+RMHD_DEV void mbar_arrive(unsigned long long* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+RMHD_DEV void mbar_wait(unsigned long long* bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "HM_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra HM_DONE;\n"
+      "bra HM_WAIT;\n"
+      "HM_DONE:\n"
+      "}\n" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
+}
+
 // reconstructions of NREC consecutive fields starting at field F0 of one face (shared memory), G at a time
 template <int F0, int NREC, int G, int DONE = 0>
 RMHD_DEV void face_recon_range(const double* p, int fs, int st, double* o) {
@@ -66,6 +86,10 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
   constexpr int TX = FF_TX, TY = FF_TY, XW = FF_XW, YR = FF_YR;
   constexpr int FSX = TY * XW, FSY = YR * TX;       // field strides of gX, gY
   extern __shared__ double sm[];
+  __shared__ unsigned long long bar2;                // "P2 done" (fY, fX written; gX, gY no longer read)
+  if (threadIdx.x == 0) mbar_init(&bar2, HM_THREADS);
+  __syncthreads();
+  unsigned ph2 = 0;
   double* gX = sm;
   double* gY = gX + SM::GX;
   double* fY = gY + SM::GY;
@@ -169,13 +193,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
             }
           }
         }
-        hm_barrier();
-#pragma unroll
-        for (int h = 0; h < NHV; ++h) Lacc[h] = fma(-fY[(FS::hv(h) * (TY + 1) + ty + 1) * TX + lane], hidy, Lacc[h]);
-        if (lane == 31) {
-#pragma unroll
-          for (int h = 0; h < NHV; ++h) Lacc[h] = fma(-fX[FS::hv(h) * TY + ty], hidx, Lacc[h]);
-        }
+        mbar_arrive(&bar2);                          // waited for after the z part
       }
       if (HAS_Z) {
         double u0[2 * NHV];
@@ -215,9 +233,18 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
         for (int f = 0; f < 2 * NHV; ++f) ring[s_old + f * FF_MAIN] = u0[f];
         { const int t = s_old; s_old = s_new; s_new = t; }
       }
-      if (do_xy && inside) {
-        const unsigned id = pk + (unsigned)j * nx + i;
-        store_rows<COMB, NHV>(L, cb, N, id, Lacc, [](int h) { return FS::hv(h); });
+      if (do_xy) {
+        mbar_wait(&bar2, ph2); ph2 ^= 1u;
+#pragma unroll
+        for (int h = 0; h < NHV; ++h) Lacc[h] = fma(-fY[(FS::hv(h) * (TY + 1) + ty + 1) * TX + lane], hidy, Lacc[h]);
+        if (lane == 31) {
+#pragma unroll
+          for (int h = 0; h < NHV; ++h) Lacc[h] = fma(-fX[FS::hv(h) * TY + ty], hidx, Lacc[h]);
+        }
+        if (inside) {
+          const unsigned id = pk + (unsigned)j * nx + i;
+          store_rows<COMB, NHV>(L, cb, N, id, Lacc, [](int h) { return FS::hv(h); });
+        }
       }
     } else {
       // ======================================= role M =======================================
@@ -322,7 +349,8 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
             for (int h = 0; h < NHV; ++h) fX[FS::hv(h) * TY + lane] = o[h] + o[NHV + h];
           }
         }
-        hm_barrier();
+        mbar_arrive(&bar2);
+        mbar_wait(&bar2, ph2); ph2 ^= 1u;
 #pragma unroll
         for (int v = 0; v < NM; ++v) Lacc[v] = fma(-fY[(hm_mrow(v) * (TY + 1) + ty + 1) * TX + lane], hidy, Lacc[v]);
         if (lane == 31) {
