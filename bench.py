@@ -243,28 +243,43 @@ def run_ours(args):
     value = world * ncell * args.steps / (ms_total * 1e-3)
 
     # ---- roofline of the dominant kernel class -------------------------------------------------
+    naxes = sum(1 for n in (nx, ny, nz) if n > 1)
     dom = max(("stage1", "stage2", "flux", "combine_c2p"), key=lambda k: kt[k]["ms"])
     avg_ms = kt[dom]["ms"] / max(kt[dom]["launches"], 1)
     shares = {k: round(v["ms"] / max(sum(x["ms"] for x in kt.values()), 1e-30), 4) for k, v in kt.items()}
-    alg_bytes = {  # SURVEY.md 8(d) table, doubles per cell per launch x 8 B (resistive)
-        "stage1": 29 * 8 * ncell, "stage2": 57 * 8 * ncell,
-        # one L(q) evaluation = 33 doubles per cell; the fused kernel does it in 1 launch, the split path in naxes
-        "flux": 33 * 8 * ncell * 2 * args.steps / max(kt["flux"]["launches"], 1),
-        "combine_c2p": 76 * 8 * ncell,   # 76 incl. the fused F2 reads; the un-fused kernel's own minimum is 62
+    # algorithmic doubles per cell per launch (resistive 14 cons + 5 prims, 5 source rows).
+    # Fused path (nx, ny > 1): stage 2 also writes A (eq 11 partial sum), F2 reads A and writes q^{n+1}, P is con2prim only.
+    fused = nx > 1 and ny > 1 and os.environ.get("RMHD_FLUX") != "split" and os.environ.get("RMHD_COMBINE") != "split"
+    nfl = max(kt["flux"]["launches"], 1) / (2.0 * args.steps)      # launches per L(q): 1 fused, naxes split
+    alg_bytes = {
+        "stage1": 34 * 8 * ncell,                                   # R qn 14 + w 5; W E*,psi*,phi* 5 + w 5 + Psi1 5
+        "stage2": (71 if fused else 62) * 8 * ncell,                # R qn 14 + L1 14 + Psi1 5 + w 5; W q2 14 + w 5 + (A 14 | Psi2 5)
+        "flux": ((33 + 47) / 2.0 if fused else 33 / nfl) * 8 * ncell,   # F1: R 19, W 14; fused F2: R 19 + A 14, W 14
+        "combine_c2p": (21 if fused else 76) * 8 * ncell,           # fused: con2prim R 11 + 5, W 5; else k_final R 57, W 19
     }
+    peak_tf = SM_COUNT * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 * 1e-12
+    alu_src = "derived: 148 SMs x 64 FP64 FMA lanes x 2 x sm_max_mhz (DESIGN.md section 5)"
     if dom in ("stage1", "stage2"):
         nsolve = stats["hist_stage"].sum()
         fl = stage_flops(stats["hist_stage"]) / max(nsolve, 1) * ncell
-        peak_tf = SM_COUNT * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 * 1e-12
         roof = {"bound": "alu", "kernel": dom, "achieved": fl / (avg_ms * 1e-3) * 1e-12, "peak": peak_tf, "unit": "TFLOP/s",
-                "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x sm_max_mhz (DESIGN.md)", "traffic": None}
+                "peak_source": alu_src, "traffic": None}
+    elif dom == "flux":
+        # The fused L(q) kernel moves its algorithmic bytes once but is bound by FP64 issue (ncu: FP64 pipe 44 % busy,
+        # DRAM 22 % of peak), so its roofline is the FP64 ALU one.  Algorithmic flops of one L(q) per cell (FMA = 2,
+        # div = 1): per axis 430 (resistive) / 628 (two-fluid) + 30 / 45 per cell.
+        per_axis, per_cell = (430.0, 30.0) if p["model"] == 0 else (628.0, 45.0)
+        fl = (per_axis * naxes + per_cell) * ncell * (2 * args.steps * 1.0 / max(kt["flux"]["launches"], 1))
+        roof = {"bound": "alu", "kernel": dom, "achieved": fl / (avg_ms * 1e-3) * 1e-12, "peak": peak_tf, "unit": "TFLOP/s",
+                "peak_source": alu_src, "traffic": None,
+                "hbm_achieved_gbs": alg_bytes[dom] / (avg_ms * 1e-3) * 1e-9, "hbm_peak_gbs": hbm_peak}
     else:
         roof = {"bound": "hbm", "kernel": dom, "achieved": alg_bytes[dom] / (avg_ms * 1e-3) * 1e-9, "peak": hbm_peak,
                 "unit": "GB/s", "peak_source": peak_src + " (MEASURED_PEAKS.json hbm_gbs)", "traffic": None}
     roof["frac"] = roof["achieved"] / roof["peak"]
     roof["avg_launch_ms"] = avg_ms
     roof["kernel_time_shares"] = shares
-    step_alg_bytes = 195 * 8 * ncell
+    step_alg_bytes = 195 * 8 * ncell          # the minimum for the step, whatever the kernel split
     roof["whole_step_hbm_frac"] = step_alg_bytes / (ms_total / args.steps * 1e-3) * 1e-9 / hbm_peak
 
     # ---- end to end through the C-ABI with host buffers ---------------------------------------
