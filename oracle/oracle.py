@@ -28,13 +28,13 @@ class OracleParams(C.Structure):
         ("gamma", C.c_double), ("sigma", C.c_double), ("eta", C.c_double), ("mu_e", C.c_double),
         ("mu_p", C.c_double), ("kappa", C.c_double), ("cfl", C.c_double), ("tol_c2p", C.c_double),
         ("tol_stage", C.c_double),
-        ("max_iter_c2p", C.c_int), ("max_iter_stage", C.c_int),
+        ("max_iter_c2p", C.c_int), ("max_iter_stage", C.c_int), ("integrator", C.c_int),
     ]
 
 
 def make_params(model=0, nx=1, ny=1, nz=1, ng=4, xlim=(0.0, 1.0), ylim=(0.0, 1.0), zlim=(0.0, 1.0),
                 bc=(0, 0, 0), gamma=4.0 / 3.0, sigma=0.0, eta=0.0, mu_e=-1.0, mu_p=1.0, kappa=1.0, cfl=0.4,
-                tol_c2p=1e-13, tol_stage=1e-12, max_iter_c2p=100, max_iter_stage=50, **_ignored):
+                tol_c2p=1e-13, tol_stage=1e-12, max_iter_c2p=100, max_iter_stage=50, integrator=0, **_ignored):
     p = OracleParams()
     p.model, p.nx, p.ny, p.nz, p.ng = model, nx, ny, nz, ng
     p.xmin, p.xmax = xlim
@@ -44,6 +44,7 @@ def make_params(model=0, nx=1, ny=1, nz=1, ng=4, xlim=(0.0, 1.0), ylim=(0.0, 1.0
     p.gamma, p.sigma, p.eta, p.mu_e, p.mu_p, p.kappa, p.cfl = gamma, sigma, eta, mu_e, mu_p, kappa, cfl
     p.tol_c2p, p.tol_stage = tol_c2p, tol_stage
     p.max_iter_c2p, p.max_iter_stage = max_iter_c2p, max_iter_stage
+    p.integrator = {"ssp2": 0, "ssp3": 1}.get(integrator, integrator)   # 2 = SSP2(222) via the general stepper (tests)
     return p
 
 

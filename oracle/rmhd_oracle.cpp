@@ -499,6 +499,7 @@ struct Sim {
   double lo[3], hi[3], dx[3];
   int bc[3];
   double cfl, dt, t0;
+  int integrator;
   long long nstep;
   size_t ntot;
   int nc, np;
@@ -669,6 +670,94 @@ void step_once(Sim& S) {
   S.nstep++;
 }
 
+// T': one step of a general IMEX Runge-Kutta scheme written exactly as eq (10)-(11) P:L152-155 (read as G1):
+//   q^(i)   = qn + dt sum_{j<i} at[i][j] L(q^(j)) + dt sum_{j<=i} a[i][j] Psi(q^(j)),   i = 1..nu
+//   q^{n+1} = qn + dt sum_j wt[j] L(q^(j)) + dt sum_j w[j] Psi(q^(j))
+// Stage i is the implicit solve q^(i) = q_ex + a[i][i] dt Psi(q^(i)) with q_ex the already known part.
+// Used for SSP3(332), Table 3 P:L174-180 (G13: the row that lost its entries is c~ = 1, a~_21 = 1), and, as a
+// cross-check of this routine against step_once, for SSP2(222), Table 2.
+struct Tableau {
+  int nu;
+  double at[3][3], wt[3];   // explicit (tilde) part
+  double a[3][3], w[3];     // implicit part
+};
+
+Tableau tableau_ssp2_222() {
+  const double g = 1.0 - 1.0 / std::sqrt(2.0);
+  Tableau T{};
+  T.nu = 2;
+  T.at[1][0] = 1.0; T.wt[0] = 0.5; T.wt[1] = 0.5;
+  T.a[0][0] = g; T.a[1][0] = 1.0 - 2.0 * g; T.a[1][1] = g; T.w[0] = 0.5; T.w[1] = 0.5;
+  return T;
+}
+
+Tableau tableau_ssp3_332() {
+  const double g = 1.0 - 1.0 / std::sqrt(2.0);
+  Tableau T{};
+  T.nu = 3;
+  T.at[1][0] = 1.0; T.at[2][0] = 0.25; T.at[2][1] = 0.25;
+  T.wt[0] = 1.0 / 6.0; T.wt[1] = 1.0 / 6.0; T.wt[2] = 2.0 / 3.0;
+  T.a[0][0] = g;
+  T.a[1][0] = 1.0 - 2.0 * g; T.a[1][1] = g;
+  T.a[2][0] = 0.5 - g; T.a[2][1] = 0.0; T.a[2][2] = g;
+  T.w[0] = 1.0 / 6.0; T.w[1] = 1.0 / 6.0; T.w[2] = 2.0 / 3.0;
+  return T;
+}
+
+void step_imex(Sim& S, const Tableau& T) {
+  const double dt = S.dt;
+  const int nc = S.nc, np = S.np;
+  const int nx = S.n[0], ny = S.n[1], nz = S.n[2];
+  const size_t a = S.ntot * nc;
+  std::vector<std::vector<double>> Ls(T.nu, std::vector<double>(a, 0.0)), Ps(T.nu, std::vector<double>(a, 0.0));
+  std::vector<double> wprev = S.w;           // Newton guess of stage i: primitives of stage i-1 (stage 1: w^n)
+  for (int st = 0; st < T.nu; ++st) {
+#pragma omp parallel for collapse(2) schedule(dynamic, 4)
+    for (int k = 0; k < nz; ++k)
+      for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i) {
+          size_t id = S.idx(i + S.g[0], j + S.g[1], k + S.g[2]);
+          long long cell = (long long)(k) * ny * nx + (long long)(j) * nx + i;
+          double qe[MAXN], wg[MAXP], qs[MAXN], ws[MAXP], ps[MAXN];
+          gather(S, S.q, nc, id, qe); gather(S, wprev, np, id, wg);
+          for (int v = 0; v < nc; ++v) {
+            size_t o = size_t(v) * S.ntot + id;
+            for (int jj = 0; jj < st; ++jj) qe[v] = qe[v] + dt * T.at[st][jj] * Ls[jj][o] + dt * T.a[st][jj] * Ps[jj][o];
+          }
+          int it, c2;
+          int rc = stage_solve(qe, wg, T.a[st][st] * dt, S.P, qs, ws, it, c2);
+          if (rc) record_fail(S, cell);
+          record(S, S.hist_stage, it); record(S, S.hist_c2p, c2);
+          source_vector(qs, ws, S.P, ps);
+          scatter(S, S.qs, nc, id, qs); scatter(S, S.w1, np, id, ws); scatter(S, Ps[st], nc, id, ps);
+        }
+    fill_ghosts(S, S.qs, nc); fill_ghosts(S, S.w1, np);
+    eval_L(S, S.qs, S.w1, Ls[st]);
+    wprev = S.w1;
+  }
+#pragma omp parallel for collapse(2) schedule(dynamic, 4)
+  for (int k = 0; k < nz; ++k)
+    for (int j = 0; j < ny; ++j)
+      for (int i = 0; i < nx; ++i) {
+        size_t id = S.idx(i + S.g[0], j + S.g[1], k + S.g[2]);
+        long long cell = (long long)(k) * ny * nx + (long long)(j) * nx + i;
+        double qn[MAXN], wg[MAXP], ws[MAXP], Zg[2], Zo[2];
+        gather(S, S.q, nc, id, qn); gather(S, wprev, np, id, wg);
+        for (int v = 0; v < nc; ++v) {
+          size_t o = size_t(v) * S.ntot + id;
+          for (int jj = 0; jj < T.nu; ++jj) qn[v] = qn[v] + dt * T.wt[jj] * Ls[jj][o] + dt * T.w[jj] * Ps[jj][o];
+        }
+        guess_Z(wg, S.P, Zg);
+        int it;
+        int rc = cons2prim(qn, S.P, Zg, ws, Zo, it);
+        if (rc) record_fail(S, cell);
+        record(S, S.hist_c2p, it);
+        scatter(S, S.q, nc, id, qn); scatter(S, S.w, np, id, ws);
+      }
+  fill_ghosts(S, S.q, nc); fill_ghosts(S, S.w, np);
+  S.nstep++;
+}
+
 }  // namespace
 
 // =====================================================================================
@@ -684,6 +773,7 @@ typedef struct {
   int bc[3];
   double gamma, sigma, eta, mu_e, mu_p, kappa, cfl, tol_c2p, tol_stage;
   int max_iter_c2p, max_iter_stage;
+  int integrator;   // 0: SSP2(222) (step_once), 1: SSP3(332) (step_imex), 2: SSP2(222) through step_imex (cross-check)
 } oracle_params;
 
 static Par to_par(const oracle_params* p) {
@@ -852,6 +942,8 @@ void* oracle_create(const oracle_params* p) {
     if (S->g[d]) inv += 1.0 / S->dx[d];
     S->ntot *= size_t(S->N[d]);
   }
+  if (p->integrator < 0 || p->integrator > 2) { delete S; return nullptr; }
+  S->integrator = p->integrator;
   S->cfl = p->cfl;
   S->dt = inv > 0 ? p->cfl / inv : p->cfl;   // G9: dt = CFL / sum_d 1/dx_d (alpha = 1)
   S->t0 = 0.0; S->nstep = 0;
@@ -934,7 +1026,10 @@ int oracle_set_cons(void* h, const double* cons, const double* prim_guess) {
 
 int oracle_step(void* h, int nsteps) {
   Sim& S = *static_cast<Sim*>(h);
-  for (int s = 0; s < nsteps; ++s) step_once(S);
+  for (int s = 0; s < nsteps; ++s) {
+    if (S.integrator == 0) step_once(S);
+    else step_imex(S, S.integrator == 1 ? tableau_ssp3_332() : tableau_ssp2_222());
+  }
   return S.n_failed ? -3 : 0;
 }
 
