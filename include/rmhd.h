@@ -30,6 +30,7 @@ typedef struct rmhd_ctx rmhd_ctx; /* opaque */
 
 enum { RMHD_RESISTIVE = 0, RMHD_TWO_FLUID = 1 };
 enum { RMHD_BC_OUTFLOW = 0, RMHD_BC_PERIODIC = 1 };
+enum { RMHD_SSP2_222 = 0, RMHD_SSP3_332 = 1 };   /* IMEX integrator: Table 2, Table 3 */
 enum {
   RMHD_OK = 0,
   RMHD_ERR_BAD_PARAM = -1,
@@ -57,6 +58,7 @@ typedef struct {
   int max_iter_c2p, max_iter_stage; /* <= 0 => 100, 50                                          */
   int device;                 /* CUDA ordinal                                                    */
   void* stream;               /* cudaStream_t owned by the caller (0 = default stream)           */
+  int integrator;             /* RMHD_SSP2_222 (default, the north-star path) | RMHD_SSP3_332     */
 } rmhd_params;
 
 /* ---- grid simulation (north_star: rmhd_create / set_initial / step / get_state / destroy) -- */
@@ -76,8 +78,9 @@ int rmhd_set_initial(rmhd_ctx* c, const double* prims, const double* rho_charge,
  * (P:L118-136); prim_guess nullable.  Used for restarts and by tests. */
 int rmhd_set_cons(rmhd_ctx* c, const double* cons, const double* prim_guess, int on_device);
 
-/* Advance nsteps full IMEX SSP2(222) steps (Table 2, eq 10-11 P:L152-155 read as
- * G1): implicit stage, L(q1), implicit stage, L(q2), combine, con2prim.  Everything runs on
+/* Advance nsteps full IMEX steps (eq 10-11 P:L152-155 read as G1).  SSP2(222), Table 2 P:L167-172:
+ * implicit stage, L(q1), implicit stage, L(q2), combine, con2prim.  SSP3(332), Table 3
+ * (reading G13): three implicit stages and three L evaluations, same kernels.  Everything runs on
  * the context's stream; one 16-byte device->host read of the failure counters at the end.
  * Returns NONCONVERGED if any root-find failed in any cell (the steps are still completed). */
 int rmhd_step(rmhd_ctx* c, int nsteps);

@@ -46,13 +46,13 @@ class rmhd_params(C.Structure):
         ("gamma", C.c_double), ("sigma", C.c_double), ("eta", C.c_double), ("mu_e", C.c_double), ("mu_p", C.c_double),
         ("kappa", C.c_double), ("cfl", C.c_double), ("tol_c2p", C.c_double), ("tol_stage", C.c_double),
         ("max_iter_c2p", C.c_int), ("max_iter_stage", C.c_int),
-        ("device", C.c_int), ("stream", C.c_void_p),
+        ("device", C.c_int), ("stream", C.c_void_p), ("integrator", C.c_int),
     ]
 
 
 def make_params(model=0, nx=1, ny=1, nz=1, ng=4, xlim=(0.0, 1.0), ylim=(0.0, 1.0), zlim=(0.0, 1.0), bc=(0, 0, 0),
                 gamma=4.0 / 3.0, sigma=0.0, eta=0.0, mu_e=-1.0, mu_p=1.0, kappa=1.0, cfl=0.4, tol_c2p=1e-13,
-                tol_stage=1e-12, max_iter_c2p=100, max_iter_stage=50, device=0, stream=None, **_ignored):
+                tol_stage=1e-12, max_iter_c2p=100, max_iter_stage=50, device=0, stream=None, integrator=0, **_ignored):
     p = rmhd_params()
     p.model, p.nx, p.ny, p.nz, p.ng = model, nx, ny, nz, ng
     p.xmin, p.xmax = xlim
@@ -63,6 +63,7 @@ def make_params(model=0, nx=1, ny=1, nz=1, ng=4, xlim=(0.0, 1.0), ylim=(0.0, 1.0
     p.tol_c2p, p.tol_stage, p.max_iter_c2p, p.max_iter_stage = tol_c2p, tol_stage, max_iter_c2p, max_iter_stage
     p.device = device
     p.stream = _current_stream(device) if stream is None else stream
+    p.integrator = {"ssp2": 0, "ssp3": 1}.get(integrator, integrator)
     return p
 
 

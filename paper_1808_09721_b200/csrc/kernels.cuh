@@ -16,6 +16,13 @@ struct Stats {
   unsigned long long n_bad_input;
 };
 
+// coefficients of one implicit stage (times dt), from the Butcher tables (Table 2, Table 3)
+struct StageCoef {
+  double a;                // a_ii dt
+  double cL[2], cP[2];     // q_ex = qn + cL0 L1 + cL1 L2 + cP0 Psi1 + cP1 Psi2            (a~_ij dt, a_ij dt)
+  double hL[2], hP[3];     // A    = qn + hL0 L1 + hL1 L2 + hP0 Psi1 + hP1 Psi2 + hP2 Psi  (w~_j dt, w_j dt)
+};
+
 template <int MODEL> struct ConsRows { const double* r[Dim<MODEL>::NC]; };
 template <int MODEL> struct HydRows { const double* r[Dim<MODEL>::NH]; };
 
@@ -166,19 +173,20 @@ __global__ void __launch_bounds__(256) k_con2prim(const double* __restrict__ con
 // =======================================================================================
 // a1: implicit stage, resistive.  One thread per cell, everything in registers; the Newton
 // loop is warp-voted so a warp leaves as soon as all its 32 cells have converged.
-//   STAGE 1: q_ex = qn.                       writes E*, psi*, phi* rows of qs, prims, Psi1
-//   STAGE 2: q_ex = qn + dt L1 + (1-2g) dt Psi1 (fused a5).  writes all rows of qs, prims, Psi2
+// Stage i of eq (10) with NL = i - 1 earlier stages (SSP2(222): NL = 0, 1; SSP3(332): NL = 0, 1, 2):
+//   NL = 0: q_ex = qn.                        writes E*, psi*, phi* rows of qs, prims, Psi
+//   NL > 0: q_ex = qn + cL0 L1 + cL1 L2 + cP0 Psi1 + cP1 Psi2 (fused a5).  writes all rows of qs, prims, Psi
 // Psi rows stored: -J (3), rhoc - kappa psi*, -kappa phi*.
-// MKA (stage 2 on the fused-flux path): instead of Psi2 the kernel writes the part of eq (11) that is known
-// once stage 2 is solved,  A_v = qn_v + hdt L1_v + hdt (Psi1_v + Psi2_v)  (all NC rows, into the buffer that
-// would have held L2), so that the F2 flux launch finishes the step with q^{n+1}_v = A_v + hdt L2_v
-// (flux_fused.cuh, FluxComb).
+// MKA (last stage): instead of Psi the kernel writes the part of eq (11) that is known once the last stage is
+// solved,  A_v = qn_v + hL0 L1_v + hL1 L2_v + hP0 Psi1_v + hP1 Psi2_v + hP2 Psi_v(this stage)  (all NC rows), so
+// that the last flux launch finishes the step with q^{n+1}_v = A_v + w~_last dt L_last,v (flux_fused.cuh, FluxComb).
 // =======================================================================================
-template <int STAGE, bool MKA = false>
+template <int NL, bool MKA = false>
 __global__ void __launch_bounds__(128, 4) k_stage_resistive(const double* __restrict__ qn, const double* __restrict__ L1,
-                                                         const double* __restrict__ Ps1, double* __restrict__ w,
+                                                         const double* __restrict__ L2, const double* __restrict__ Ps1,
+                                                         const double* __restrict__ Ps2, double* __restrict__ w,
                                                          double* __restrict__ qs, double* __restrict__ Ps, double* __restrict__ A,
-                                                         size_t N, double a, double cL, double cP, double hdt, DevPar P, Stats* st) {
+                                                         size_t N, StageCoef k, DevPar P, Stats* st) {
   __shared__ int shist[NBINS];
   BlockHist bh; bh.init(shist);
   const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -190,20 +198,31 @@ __global__ void __launch_bounds__(128, 4) k_stage_resistive(const double* __rest
     double qe[R_NC];
 #pragma unroll
     for (int v = 0; v < R_NC; ++v) qe[v] = qn[(size_t)v * N + c];
-    if (STAGE == 2) {
+    if (NL >= 1) {
 #pragma unroll
       for (int v = 0; v < R_NC; ++v) {
-        const double l = L1[(size_t)v * N + c];
-        if (MKA && (v < 8 || v == 11)) A[(size_t)v * N + c] = fma(hdt, l, qe[v]);
-        qe[v] = fma(cL, l, qe[v]);
+        double av = qe[v];
+        const double l1 = L1[(size_t)v * N + c];
+        if (MKA) av = fma(k.hL[0], l1, av);
+        qe[v] = fma(k.cL[0], l1, qe[v]);
+        if (NL >= 2) {
+          const double l2 = L2[(size_t)v * N + c];
+          if (MKA) av = fma(k.hL[1], l2, av);
+          qe[v] = fma(k.cL[1], l2, qe[v]);
+        }
+        if (MKA && (v < 8 || v == 11)) A[(size_t)v * N + c] = av;
       }
-      qe[8] += cP * Ps1[0 * N + c]; qe[9] += cP * Ps1[1 * N + c]; qe[10] += cP * Ps1[2 * N + c];
-      qe[12] += cP * Ps1[3 * N + c]; qe[13] += cP * Ps1[4 * N + c];
+#pragma unroll
+      for (int j = 0; j < R_NS; ++j) {
+        const int v = j < 3 ? 8 + j : 9 + j;
+        qe[v] = fma(k.cP[0], Ps1[(size_t)j * N + c], qe[v]);
+        if (NL >= 2 && k.cP[1] != 0.0) qe[v] = fma(k.cP[1], Ps2[(size_t)j * N + c], qe[v]);
+      }
 #pragma unroll
       for (int v = 0; v < R_NC; ++v) if (v < 8 || v == 11) qs[(size_t)v * N + c] = qe[v];
     }
     qpsi = qe[12]; qphi = qe[13];
-    r_stage_init(s, qe, w[c], w[N + c], w[2 * N + c], w[3 * N + c], w[4 * N + c], a, P.sigma, P);
+    r_stage_init(s, qe, w[c], w[N + c], w[2 * N + c], w[3 * N + c], w[4 * N + c], k.a, P.sigma, P);
   }
   while (true) {
     const bool active = s.status == 0 && s.iters < P.maxit_stage;
@@ -213,11 +232,13 @@ __global__ void __launch_bounds__(128, 4) k_stage_resistive(const double* __rest
   if (valid) {
     Hyd h; double J[3], psi, phi;
     double Ap[R_NS];
-    if (MKA) {       // qn, L1, Psi1 of the source rows again (L2 hits) rather than 10 registers held across the Newton loop
+    if (MKA) {       // qn, L, Psi of the source rows again (L2 hits) rather than 10 registers held across the Newton loop
 #pragma unroll
-      for (int k = 0; k < R_NS; ++k) {
-        const size_t v = k < 3 ? 8 + k : 9 + k;
-        Ap[k] = fma(hdt, L1[v * N + c] + Ps1[(size_t)k * N + c], qn[v * N + c]);
+      for (int j = 0; j < R_NS; ++j) {
+        const size_t v = j < 3 ? 8 + j : 9 + j;
+        double av = fma(k.hL[0], L1[v * N + c], fma(k.hP[0], Ps1[(size_t)j * N + c], qn[v * N + c]));
+        if (NL >= 2) av = fma(k.hL[1], L2[v * N + c], fma(k.hP[1], Ps2[(size_t)j * N + c], av));
+        Ap[j] = av;
       }
     }
     r_stage_finish(s, P, h, J, psi, phi, qpsi, qphi);
@@ -225,9 +246,9 @@ __global__ void __launch_bounds__(128, 4) k_stage_resistive(const double* __rest
     w[c] = h.rho; w[N + c] = h.vx; w[2 * N + c] = h.vy; w[3 * N + c] = h.vz; w[4 * N + c] = h.p;
     const double ps[R_NS] = {-J[0], -J[1], -J[2], s.rhoc - P.kappa * psi, -P.kappa * phi};
 #pragma unroll
-    for (int k = 0; k < R_NS; ++k) {
-      if (MKA) A[(size_t)(k < 3 ? 8 + k : 9 + k) * N + c] = fma(hdt, ps[k], Ap[k]);
-      else Ps[(size_t)k * N + c] = ps[k];
+    for (int j = 0; j < R_NS; ++j) {
+      if (MKA) A[(size_t)(j < 3 ? 8 + j : 9 + j) * N + c] = fma(k.hP[2], ps[j], Ap[j]);
+      else Ps[(size_t)j * N + c] = ps[j];
     }
     bh.add(s.iters);
     if (s.status != 1 || !(h.p > 0.0) || !(h.rho > 0.0)) record_fail(st, (long long)c);
@@ -276,11 +297,12 @@ __global__ void __launch_bounds__(128) k_stage_batch_resistive(const double* __r
 // a1: implicit stage, two-fluid (same launch shape and warp-voted loop as the resistive one).
 // Source rows (Psi storage order): Sbar(3), taubar, E(3), psi, phi  = cons rows 6..9, 13..17.
 // =======================================================================================
-template <int STAGE, bool MKA = false>
+template <int NL, bool MKA = false>
 __global__ void __launch_bounds__(128) k_stage_two_fluid(const double* __restrict__ qn, const double* __restrict__ L1,
-                                                         const double* __restrict__ Ps1, double* __restrict__ w,
+                                                         const double* __restrict__ L2, const double* __restrict__ Ps1,
+                                                         const double* __restrict__ Ps2, double* __restrict__ w,
                                                          double* __restrict__ qs, double* __restrict__ Ps, double* __restrict__ A,
-                                                         size_t N, double a, double cL, double cP, double hdt, DevPar P, Stats* st) {
+                                                         size_t N, StageCoef k, DevPar P, Stats* st) {
   __shared__ int shist[NBINS];
   BlockHist bh; bh.init(shist);
   const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -292,22 +314,33 @@ __global__ void __launch_bounds__(128) k_stage_two_fluid(const double* __restric
     double qe[T_NC], wg[T_NH];
 #pragma unroll
     for (int v = 0; v < T_NC; ++v) qe[v] = qn[(size_t)v * N + c];
-    if (STAGE == 2) {
+    if (NL >= 1) {
 #pragma unroll
       for (int v = 0; v < T_NC; ++v) {
-        const double l = L1[(size_t)v * N + c];
-        if (MKA && (v < 6 || (v >= 10 && v < 13))) A[(size_t)v * N + c] = fma(hdt, l, qe[v]);
-        qe[v] = fma(cL, l, qe[v]);
+        double av = qe[v];
+        const double l1 = L1[(size_t)v * N + c];
+        if (MKA) av = fma(k.hL[0], l1, av);
+        qe[v] = fma(k.cL[0], l1, qe[v]);
+        if (NL >= 2) {
+          const double l2 = L2[(size_t)v * N + c];
+          if (MKA) av = fma(k.hL[1], l2, av);
+          qe[v] = fma(k.cL[1], l2, qe[v]);
+        }
+        if (MKA && (v < 6 || (v >= 10 && v < 13))) A[(size_t)v * N + c] = av;
       }
 #pragma unroll
-      for (int k = 0; k < T_NS; ++k) qe[k < 4 ? 6 + k : 9 + k] += cP * Ps1[(size_t)k * N + c];
+      for (int j = 0; j < T_NS; ++j) {
+        const int v = j < 4 ? 6 + j : 9 + j;
+        qe[v] = fma(k.cP[0], Ps1[(size_t)j * N + c], qe[v]);
+        if (NL >= 2 && k.cP[1] != 0.0) qe[v] = fma(k.cP[1], Ps2[(size_t)j * N + c], qe[v]);
+      }
 #pragma unroll
       for (int v = 0; v < T_NC; ++v) if (v < 6 || (v >= 10 && v < 13)) qs[(size_t)v * N + c] = qe[v];
     }
     qpsi = qe[16]; qphi = qe[17];
 #pragma unroll
     for (int v = 0; v < T_NH; ++v) wg[v] = w[(size_t)v * N + c];
-    t_stage_init(s, qe, wg, a, P);
+    t_stage_init(s, qe, wg, k.a, P);
   }
   while (true) {
     const bool active = s.status == 0 && s.iters < P.maxit_stage;
@@ -323,11 +356,13 @@ __global__ void __launch_bounds__(128) k_stage_two_fluid(const double* __restric
 #pragma unroll
     for (int v = 0; v < T_NH; ++v) w[(size_t)v * N + c] = wl[v];
 #pragma unroll
-    for (int k = 0; k < T_NS; ++k) {
+    for (int j = 0; j < T_NS; ++j) {
       if (MKA) {
-        const size_t v = k < 4 ? 6 + k : 9 + k;
-        A[v * N + c] = fma(hdt, src[k], fma(hdt, L1[v * N + c] + Ps1[(size_t)k * N + c], qn[v * N + c]));
-      } else Ps[(size_t)k * N + c] = src[k];
+        const size_t v = j < 4 ? 6 + j : 9 + j;
+        double av = fma(k.hL[0], L1[v * N + c], fma(k.hP[0], Ps1[(size_t)j * N + c], qn[v * N + c]));
+        if (NL >= 2) av = fma(k.hL[1], L2[v * N + c], fma(k.hP[1], Ps2[(size_t)j * N + c], av));
+        A[v * N + c] = fma(k.hP[2], src[j], av);
+      } else Ps[(size_t)j * N + c] = src[j];
     }
     bh.add(s.iters);
     if (s.status != 1 || !(wl[0] > 0.0) || !(wl[4] > 0.0) || !(wl[5] > 0.0) || !(wl[9] > 0.0)) record_fail(st, (long long)c);
@@ -647,6 +682,32 @@ __global__ void __launch_bounds__(256) k_final(double* __restrict__ q, const dou
     for (int v = 0; v < NC; ++v) q[(size_t)v * N + c] = ql[v];
 #pragma unroll
     for (int v = 0; v < NH; ++v) w[(size_t)v * N + c] = wl[v];
+    bh.add(it);
+    if (rc) record_fail(st, (long long)c);
+  }
+  bh.flush(st->hist_c2p);
+}
+
+// last-stage combine for the per-axis flux path when A (see StageCoef) is in use: q^{n+1} = A + wl L_last, then con2prim
+template <int MODEL>
+__global__ void __launch_bounds__(256) k_final_A(double* __restrict__ q, const double* __restrict__ A, const double* __restrict__ Ll,
+                                                 double* __restrict__ w, size_t N, double wl, DevPar P, Stats* st) {
+  constexpr int NC = Dim<MODEL>::NC, NH = Dim<MODEL>::NH;
+  __shared__ int shist[NBINS];
+  BlockHist bh; bh.init(shist);
+  const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c < N) {
+    double ql[NC], wg[NH], wo[NH];
+#pragma unroll
+    for (int v = 0; v < NC; ++v) ql[v] = fma(wl, Ll[(size_t)v * N + c], A[(size_t)v * N + c]);
+#pragma unroll
+    for (int v = 0; v < NH; ++v) wg[v] = w[(size_t)v * N + c];
+    int it;
+    const int rc = cell_con2prim<MODEL>(ql, wg, true, P, wo, it);
+#pragma unroll
+    for (int v = 0; v < NC; ++v) q[(size_t)v * N + c] = ql[v];
+#pragma unroll
+    for (int v = 0; v < NH; ++v) w[(size_t)v * N + c] = wo[v];
     bh.add(it);
     if (rc) record_fail(st, (long long)c);
   }

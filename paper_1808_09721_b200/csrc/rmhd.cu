@@ -34,7 +34,7 @@ struct rmhd_ctx {
   long long nsteps;
   int device;
   cudaStream_t stream;
-  double *q, *w, *qs, *L1, *L2, *Ps1, *Ps2;
+  double *q, *w, *qs, *L1, *L2, *Ps1, *Ps2, *A;   // A: eq-(11) partial sum, SSP3(332) only (SSP2 keeps it in L2)
   Stats* d_stats;
   Stats* h_stats;  // pinned
   bool profiling;
@@ -218,44 +218,87 @@ int launch_flux(rmhd_ctx* c, const double* qa, const double* qb, bool mix, const
   return RMHD_OK;
 }
 
+template <int MODEL, int NL, bool MKA>
+int launch_stage(rmhd_ctx* c, int cls, const StageCoef& k, double* Ps_out, double* A) {
+  const unsigned nb = blocks_for(c->N, 128);
+  Timed t(c, cls);
+  if (MODEL == 0) k_stage_resistive<NL, MKA><<<nb, 128, 0, c->stream>>>(c->q, c->L1, c->L2, c->Ps1, c->Ps2, c->w, c->qs, Ps_out, A, c->N, k, c->P, c->d_stats);
+  else k_stage_two_fluid<NL, MKA><<<nb, 128, 0, c->stream>>>(c->q, c->L1, c->L2, c->Ps1, c->Ps2, c->w, c->qs, Ps_out, A, c->N, k, c->P, c->d_stats);
+  CK(c, cudaGetLastError());
+  return RMHD_OK;
+}
+
+template <int MODEL>
+int launch_con2prim(rmhd_ctx* c) {   // P: w^{n+1} = con2prim(q^{n+1}), guess = the last stage's primitives
+  Timed t(c, KC_FINAL);
+  k_con2prim<MODEL><<<blocks_for(c->N, 256), 256, 0, c->stream>>>(c->q, c->w, c->N, c->w, c->N, nullptr, nullptr, nullptr, c->N, c->P, c->d_stats);
+  CK(c, cudaGetLastError());
+  return RMHD_OK;
+}
+
+// one SSP2(222) step, Table 2
 template <int MODEL>
 int step_once(rmhd_ctx* c) {
   const double g = 1.0 - 1.0 / sqrt(2.0);
   const double dt = c->dt;
-  const unsigned nb = blocks_for(c->N, 128);
   int rc;
-  {
-    Timed t(c, KC_STAGE1);
-    if (MODEL == 0) k_stage_resistive<1><<<nb, 128, 0, c->stream>>>(c->q, nullptr, nullptr, c->w, c->qs, c->Ps1, nullptr, c->N, g * dt, 0.0, 0.0, 0.0, c->P, c->d_stats);
-    else k_stage_two_fluid<1><<<nb, 128, 0, c->stream>>>(c->q, nullptr, nullptr, c->w, c->qs, c->Ps1, nullptr, c->N, g * dt, 0.0, 0.0, 0.0, c->P, c->d_stats);
-    CK(c, cudaGetLastError());
-  }
+  StageCoef k1 = {};
+  k1.a = g * dt;
+  if ((rc = launch_stage<MODEL, 0, false>(c, KC_STAGE1, k1, c->Ps1, nullptr))) return rc;
   if ((rc = launch_flux<MODEL>(c, c->q, c->qs, true, c->w, c->L1))) return rc;
   const bool fuse_c = uses_fused_flux(c) && c->fuse_combine;
-  {
-    Timed t(c, KC_STAGE2);
-    if (fuse_c) {   // stage 2 leaves A = qn + dt/2 L1 + dt/2 (Psi1 + Psi2) in the L2 buffer
-      if (MODEL == 0) k_stage_resistive<2, true><<<nb, 128, 0, c->stream>>>(c->q, c->L1, c->Ps1, c->w, c->qs, c->Ps2, c->L2, c->N, g * dt, dt, (1.0 - 2.0 * g) * dt, 0.5 * dt, c->P, c->d_stats);
-      else k_stage_two_fluid<2, true><<<nb, 128, 0, c->stream>>>(c->q, c->L1, c->Ps1, c->w, c->qs, c->Ps2, c->L2, c->N, g * dt, dt, (1.0 - 2.0 * g) * dt, 0.5 * dt, c->P, c->d_stats);
-    } else {
-      if (MODEL == 0) k_stage_resistive<2><<<nb, 128, 0, c->stream>>>(c->q, c->L1, c->Ps1, c->w, c->qs, c->Ps2, nullptr, c->N, g * dt, dt, (1.0 - 2.0 * g) * dt, 0.0, c->P, c->d_stats);
-      else k_stage_two_fluid<2><<<nb, 128, 0, c->stream>>>(c->q, c->L1, c->Ps1, c->w, c->qs, c->Ps2, nullptr, c->N, g * dt, dt, (1.0 - 2.0 * g) * dt, 0.0, c->P, c->d_stats);
-    }
-    CK(c, cudaGetLastError());
-  }
+  StageCoef k2 = {};
+  k2.a = g * dt; k2.cL[0] = dt; k2.cP[0] = (1.0 - 2.0 * g) * dt;
+  k2.hL[0] = 0.5 * dt; k2.hP[0] = 0.5 * dt; k2.hP[2] = 0.5 * dt;
   if (fuse_c) {
-    // F2 + C in one launch (q^{n+1} = A + dt/2 L2 row by row in the flux kernel's epilogue), then P: con2prim of q^{n+1}
+    // stage 2 leaves A = qn + dt/2 L1 + dt/2 (Psi1 + Psi2) in the L2 buffer; F2 + C in one launch
+    // (q^{n+1} = A + dt/2 L2 row by row in the flux kernel's epilogue), then P
+    if ((rc = launch_stage<MODEL, 1, true>(c, KC_STAGE2, k2, nullptr, c->L2))) return rc;
     const FluxComb cb = {c->q, c->L2, 0.5 * dt};
     if ((rc = launch_flux<MODEL>(c, c->qs, nullptr, false, c->w, c->L2, &cb))) return rc;
-    Timed t(c, KC_FINAL);
-    k_con2prim<MODEL><<<blocks_for(c->N, 256), 256, 0, c->stream>>>(c->q, c->w, c->N, c->w, c->N, nullptr, nullptr, nullptr, c->N, c->P, c->d_stats);
-    CK(c, cudaGetLastError());
-    return RMHD_OK;
+    return launch_con2prim<MODEL>(c);
   }
+  if ((rc = launch_stage<MODEL, 1, false>(c, KC_STAGE2, k2, c->Ps2, nullptr))) return rc;
   if ((rc = launch_flux<MODEL>(c, c->qs, nullptr, false, c->w, c->L2))) return rc;
   {
     Timed t(c, KC_FINAL);
     k_final<MODEL><<<blocks_for(c->N, 256), 256, 0, c->stream>>>(c->q, c->L1, c->L2, c->Ps1, c->Ps2, c->w, c->N, 0.5 * dt, c->P, c->d_stats);
+    CK(c, cudaGetLastError());
+  }
+  return RMHD_OK;
+}
+
+// one SSP3(332) step, Table 3 P:L174-180 (reading G13):
+//   S1 q1 = qn + g dt Psi1;  F1;  S2 q2 = qn + dt L1 + (1-2g) dt Psi1 + g dt Psi2;  F2;
+//   S3 q3 = qn + dt/4 (L1 + L2) + (1/2-g) dt Psi1 + g dt Psi3, which also leaves
+//      A = qn + dt/6 (L1 + L2) + dt/6 (Psi1 + Psi2) + 2dt/3 Psi3;   F3 + C: q^{n+1} = A + 2dt/3 L3;   P
+template <int MODEL>
+int step_once_ssp3(rmhd_ctx* c) {
+  const double g = 1.0 - 1.0 / sqrt(2.0);
+  const double dt = c->dt;
+  int rc;
+  StageCoef k1 = {};
+  k1.a = g * dt;
+  if ((rc = launch_stage<MODEL, 0, false>(c, KC_STAGE1, k1, c->Ps1, nullptr))) return rc;
+  if ((rc = launch_flux<MODEL>(c, c->q, c->qs, true, c->w, c->L1))) return rc;
+  StageCoef k2 = {};
+  k2.a = g * dt; k2.cL[0] = dt; k2.cP[0] = (1.0 - 2.0 * g) * dt;
+  if ((rc = launch_stage<MODEL, 1, false>(c, KC_STAGE2, k2, c->Ps2, nullptr))) return rc;
+  if ((rc = launch_flux<MODEL>(c, c->qs, nullptr, false, c->w, c->L2))) return rc;
+  StageCoef k3 = {};
+  k3.a = g * dt; k3.cL[0] = 0.25 * dt; k3.cL[1] = 0.25 * dt; k3.cP[0] = (0.5 - g) * dt; k3.cP[1] = 0.0;
+  k3.hL[0] = dt / 6.0; k3.hL[1] = dt / 6.0; k3.hP[0] = dt / 6.0; k3.hP[1] = dt / 6.0; k3.hP[2] = 2.0 * dt / 3.0;
+  if ((rc = launch_stage<MODEL, 2, true>(c, KC_STAGE2, k3, nullptr, c->A))) return rc;
+  const double wl = 2.0 * dt / 3.0;
+  if (uses_fused_flux(c) && c->fuse_combine) {
+    const FluxComb cb = {c->q, c->A, wl};
+    if ((rc = launch_flux<MODEL>(c, c->qs, nullptr, false, c->w, c->L1, &cb))) return rc;
+    return launch_con2prim<MODEL>(c);
+  }
+  if ((rc = launch_flux<MODEL>(c, c->qs, nullptr, false, c->w, c->L1))) return rc;   // L3 into the L1 buffer (L1 is folded into A)
+  {
+    Timed t(c, KC_FINAL);
+    k_final_A<MODEL><<<blocks_for(c->N, 256), 256, 0, c->stream>>>(c->q, c->A, c->L1, c->w, c->N, wl, c->P, c->d_stats);
     CK(c, cudaGetLastError());
   }
   return RMHD_OK;
@@ -286,6 +329,7 @@ int rmhd_create(const rmhd_params* p, rmhd_ctx** out) {
   DevPar P;
   int rc = make_devpar(p, P, g_create_error);
   if (rc) return rc;
+  if (p->integrator != RMHD_SSP2_222 && p->integrator != RMHD_SSP3_332) { g_create_error = "integrator must be RMHD_SSP2_222 or RMHD_SSP3_332"; return RMHD_ERR_BAD_PARAM; }
   if (p->nx < 1 || p->ny < 1 || p->nz < 1 || p->ng < 2 || !(p->cfl > 0.0)) { g_create_error = "bad grid size, ng < 2 or cfl <= 0"; return RMHD_ERR_BAD_PARAM; }
   for (int d = 0; d < 3; ++d) if (p->bc[d] != RMHD_BC_OUTFLOW && p->bc[d] != RMHD_BC_PERIODIC) { g_create_error = "bad boundary condition"; return RMHD_ERR_BAD_PARAM; }
   int ndev = 0;
@@ -318,10 +362,10 @@ int rmhd_create(const rmhd_params* p, rmhd_ctx** out) {
   { const char* e = getenv("RMHD_COMBINE"); c->fuse_combine = !(e && strcmp(e, "split") == 0); }
   c->sm_count = 148;
   for (int i = 0; i < KC_N; ++i) { c->ms[i] = 0.0; c->launches[i] = 0; }
-  c->q = c->w = c->qs = c->L1 = c->L2 = c->Ps1 = c->Ps2 = nullptr; c->d_stats = nullptr; c->h_stats = nullptr;
+  c->q = c->w = c->qs = c->L1 = c->L2 = c->Ps1 = c->Ps2 = c->A = nullptr; c->d_stats = nullptr; c->h_stats = nullptr;
   DeviceGuard dg(c->device);
   { int n = 0; if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, c->device) == cudaSuccess && n > 0) c->sm_count = n; }
-  const size_t rows = (size_t)(4 * c->nc + c->nh + 2 * c->ns);
+  const size_t rows = (size_t)((p->integrator == RMHD_SSP3_332 ? 5 : 4) * c->nc + c->nh + 2 * c->ns);
   cudaError_t e = cudaMalloc(&c->q, sizeof(double) * rows * c->N);
   if (e == cudaSuccess) e = cudaMalloc(&c->d_stats, sizeof(Stats));
   if (e == cudaSuccess) e = cudaMallocHost(&c->h_stats, sizeof(Stats));
@@ -333,6 +377,7 @@ int rmhd_create(const rmhd_params* p, rmhd_ctx** out) {
   b += (size_t)c->nc * c->N; c->w = b;
   b += (size_t)c->nh * c->N; c->Ps1 = b;
   b += (size_t)c->ns * c->N; c->Ps2 = b;
+  if (p->integrator == RMHD_SSP3_332) { b += (size_t)c->ns * c->N; c->A = b; }
   e = cudaMemsetAsync(c->q, 0, sizeof(double) * rows * c->N, c->stream);
   if (e != cudaSuccess) { fail_cuda(nullptr, e, "clearing device state"); rmhd_destroy(c); return RMHD_ERR_CUDA; }
   if (reset_stats(c)) { g_create_error = c->err; rmhd_destroy(c); return RMHD_ERR_CUDA; }
@@ -411,7 +456,9 @@ int rmhd_step(rmhd_ctx* c, int nsteps) {
   if (!c || nsteps < 0) return RMHD_ERR_BAD_PARAM;
   DeviceGuard dg(c->device);
   for (int s = 0; s < nsteps; ++s) {
-    int rc = c->model == 0 ? step_once<0>(c) : step_once<1>(c);
+    int rc;
+    if (c->p.integrator == RMHD_SSP3_332) rc = c->model == 0 ? step_once_ssp3<0>(c) : step_once_ssp3<1>(c);
+    else rc = c->model == 0 ? step_once<0>(c) : step_once<1>(c);
     if (rc) return rc;
     c->nsteps++;
   }

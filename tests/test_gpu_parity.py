@@ -348,3 +348,34 @@ def test_set_cons_get_state_round_trip_and_device_buffers(B, O, synth):
     sim2 = B.Rmhd(**c["params"]); assert sim2.set_cons(q, w) == 0; sim2.step(2); q5b, _ = sim2.get_state(); sim2.close()
     assert rel_l1(q5b, q5) < 1e-13
     assert abs(B.Rmhd(**c["params"]).dt - 0.4 / (32 / 1.0 + 24 / 2.0)) < 1e-16
+
+
+# ------------------------------------------------------------------------------------------
+# SSP3(332) (Table 3): same kernels, three stages
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("case", ["tube_1d", "shear_2d", "blast_3d", "two_fluid_2d", "blast_3d_split"])
+def test_ssp3_332_parity(B, O, synth, case, monkeypatch):
+    if case == "tube_1d":                 # per-axis flux kernels + k_final_A
+        c = synth.config1(); nsteps, tol = 128, 1e-9
+    elif case == "shear_2d":              # fused two-role flux kernel, 2-D, partial tiles
+        c = synth.config3(nx=80, ny=72, nsteps=40); nsteps, tol = 40, 1e-8
+    elif case in ("blast_3d", "blast_3d_split"):
+        c = synth.config5(n=40, nsteps=12); nsteps, tol = 12, 1e-8
+        if case == "blast_3d_split":
+            monkeypatch.setenv("RMHD_FLUX", "split")
+    else:
+        c = synth.config4(nx=48, ny=40, nsteps=30); nsteps, tol = 30, 1e-8
+    q, w, st = run_gpu(B, c, nsteps=nsteps, params_override={"integrator": "ssp3"})
+    qo, wo, _ = run_oracle(O, c, nsteps=nsteps, params_override={"integrator": "ssp3"})
+    assert st["n_failed"] == 0
+    assert rel_l1(q, qo) <= tol, rel_l1(q, qo)
+    ncell = int(np.prod(c["prims"].shape[1:]))
+    assert st["hist_stage"].sum() == 3 * ncell * nsteps and st["hist_c2p"].sum() == ncell * nsteps
+    # and it is a different scheme from SSP2(222)
+    q2, _, _ = run_gpu(B, c, nsteps=nsteps)
+    assert rel_l1(q2, qo) > 1e-7
+
+
+def test_bad_integrator_is_rejected(B):
+    with pytest.raises(B.RmhdError):
+        B.Rmhd(model=0, nx=8, integrator=7)
