@@ -1,12 +1,13 @@
 #!/usr/bin/env python
 """bench.py -- throughput of one full IMEX SSP2(222) step (all SURVEY.md 8(a) rows) on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg5|cfg2|...]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg5|cfg3|cfg4|cfg1]
+                    [--integrator ssp2|ssp3]
 
 Workload at N=1: BASELINE.json configs[4], the 3-D 256^3 resistive blast -- the configuration
 the metric ("FP64 zone-updates/s per full IMEX step") and the north-star target are quoted on;
-configs[1] is a single implicit stage, not a full step, so it is a parity case and an optional
-`--workload cfg2` line, not the headline.  Inputs are synthetic (paper_1808_09721_b200.synth).
+configs[1] is a single implicit stage, not a full step, so it is a parity case, not a bench line.
+`--integrator ssp3` times the SSP3(332) step on the same workloads; the headline is SSP2(222).  Inputs are synthetic (paper_1808_09721_b200.synth).
 Prints ONE JSON line (rank 0).  Multi-GPU: the path does not shard in this build ("replicas
 only"): each rank steps its own copy; value = zone-updates of all ranks / max time.
 
@@ -133,9 +134,10 @@ def oracle_sample(cfg, synth):
     return p, w, what
 
 
-def time_oracle(cfg, synth, steps, warmup, budget_s=40.0):
+def time_oracle(cfg, synth, steps, warmup, budget_s=40.0, integrator="ssp2"):
     from oracle import oracle as O
     p, w, what = oracle_sample(cfg, synth)
+    p["integrator"] = integrator
     cores = O.set_threads(0)
     S = O.OracleSim(O.make_params(**p))
     S.set_initial(w, cfg.get("rho_charge"))
@@ -165,7 +167,7 @@ def run_reference(args):
         return
     from paper_1808_09721_b200 import synth
     cfg = make_workload(args.workload, synth)
-    base, ms, done = time_oracle(cfg, synth, args.steps, min(args.warmup, 1), budget_s=120.0)
+    base, ms, done = time_oracle(cfg, synth, args.steps, min(args.warmup, 1), budget_s=120.0, integrator=args.integrator)
     line = {
         "impl": "reference", "metric": METRIC, "value": base["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": done,
         "warmup": min(args.warmup, 1), "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -206,7 +208,8 @@ def run_ours(args):
     dev = torch.device("cuda", local)
 
     cfg = make_workload(args.workload, synth)
-    p = dict(cfg["params"]); p["device"] = local
+    p = dict(cfg["params"]); p["device"] = local; p["integrator"] = args.integrator
+    nstage = 3 if args.integrator == "ssp3" else 2
     nz, ny, nx = cfg["prims"].shape[1:]
     ncell = nx * ny * nz
     sim = B.Rmhd(**p)
@@ -250,11 +253,11 @@ def run_ours(args):
     # algorithmic doubles per cell per launch (resistive 14 cons + 5 prims, 5 source rows).
     # Fused path (nx, ny > 1): stage 2 also writes A (eq 11 partial sum), F2 reads A and writes q^{n+1}, P is con2prim only.
     fused = nx > 1 and ny > 1 and os.environ.get("RMHD_FLUX") != "split" and os.environ.get("RMHD_COMBINE") != "split"
-    nfl = max(kt["flux"]["launches"], 1) / (2.0 * args.steps)      # launches per L(q): 1 fused, naxes split
+    nfl = max(kt["flux"]["launches"], 1) / (float(nstage) * args.steps)   # launches per L(q): 1 fused, naxes split
     alg_bytes = {
         "stage1": 34 * 8 * ncell,                                   # R qn 14 + w 5; W E*,psi*,phi* 5 + w 5 + Psi1 5
         "stage2": (71 if fused else 62) * 8 * ncell,                # R qn 14 + L1 14 + Psi1 5 + w 5; W q2 14 + w 5 + (A 14 | Psi2 5)
-        "flux": ((33 + 47) / 2.0 if fused else 33 / nfl) * 8 * ncell,   # F1: R 19, W 14; fused F2: R 19 + A 14, W 14
+        "flux": ((33 * (nstage - 1) + 47) / float(nstage) if fused else 33 / nfl) * 8 * ncell,   # F: R 19, W 14; fused last F: R 19 + A 14, W 14
         "combine_c2p": (21 if fused else 76) * 8 * ncell,           # fused: con2prim R 11 + 5, W 5; else k_final R 57, W 19
     }
     peak_tf = SM_COUNT * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 * 1e-12
@@ -269,7 +272,7 @@ def run_ours(args):
         # DRAM 22 % of peak), so its roofline is the FP64 ALU one.  Algorithmic flops of one L(q) per cell (FMA = 2,
         # div = 1): per axis 430 (resistive) / 628 (two-fluid) + 30 / 45 per cell.
         per_axis, per_cell = (430.0, 30.0) if p["model"] == 0 else (628.0, 45.0)
-        fl = (per_axis * naxes + per_cell) * ncell * (2 * args.steps * 1.0 / max(kt["flux"]["launches"], 1))
+        fl = (per_axis * naxes + per_cell) * ncell * (nstage * args.steps * 1.0 / max(kt["flux"]["launches"], 1))
         roof = {"bound": "alu", "kernel": dom, "achieved": fl / (avg_ms * 1e-3) * 1e-12, "peak": peak_tf, "unit": "TFLOP/s",
                 "peak_source": alu_src, "traffic": None,
                 "hbm_achieved_gbs": alg_bytes[dom] / (avg_ms * 1e-3) * 1e-9, "hbm_peak_gbs": hbm_peak}
@@ -279,7 +282,9 @@ def run_ours(args):
     roof["frac"] = roof["achieved"] / roof["peak"]
     roof["avg_launch_ms"] = avg_ms
     roof["kernel_time_shares"] = shares
-    step_alg_bytes = 195 * 8 * ncell          # the minimum for the step, whatever the kernel split
+    # the minimum for the SSP2(222) step, whatever the kernel split; SSP3(332) by the same rules:
+    # S1 29 + F1 33 + S2 57 + F2 33 + S3 76 + (F3 + C + P fused) 95
+    step_alg_bytes = (323 if nstage == 3 else 195) * 8 * ncell
     roof["whole_step_hbm_frac"] = step_alg_bytes / (ms_total / args.steps * 1e-3) * 1e-9 / hbm_peak
 
     # ---- end to end through the C-ABI with host buffers ---------------------------------------
@@ -315,14 +320,14 @@ def run_ours(args):
         return
     cpu_base = None
     if world == 1 and not args.no_cpu_baseline:
-        cpu_base, _, _ = time_oracle(cfg, synth, steps=12, warmup=0, budget_s=20.0)
+        cpu_base, _, _ = time_oracle(cfg, synth, steps=12, warmup=0, budget_s=20.0, integrator=args.integrator)
     launches = sum(v["launches"] for v in kt.values())
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": f"{cfg['name']}: {nx}x{ny}x{nz} cells, {'resistive' if p['model'] == 0 else 'two_fluid'}, "
-                               f"SSP2(222), cfl {p['cfl']}, sigma {p.get('sigma')}",
+                               f"{'SSP3(332)' if nstage == 3 else 'SSP2(222)'}, cfl {p['cfl']}, sigma {p.get('sigma')}",
                    "parallelism": "replicas only" if world > 1 else "1 gpu",
                    "l2": "state arrays (%.1f GB) exceed the 126 MB L2; no flush needed" % (71 * ncell * 8 / 1e9),
                    "n_failed_cells": int(n_failed),
@@ -342,6 +347,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg5")
+    ap.add_argument("--integrator", default="ssp2", choices=["ssp2", "ssp3"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
