@@ -103,7 +103,7 @@ def test_prim2cons_con2prim_batch_two_fluid(B, O, synth):
 # ------------------------------------------------------------------------------------------
 # config 2: batched implicit stage
 # ------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("n", [1, 31, 2 ** 16 + 37])
+@pytest.mark.parametrize("n", [1, 31, 2 ** 16 + 37, 2 ** 20])      # 2^20 = BASELINE.json configs[1] in full
 def test_config2_stage_batch_parity(B, O, synth, n):
     c = synth.config2(n, seed=0)
     P = B.make_params(**c["params"]); PO = O.make_params(**c["params"])
@@ -235,6 +235,18 @@ def test_config1_riemann_tube_full(B, O, synth):
 
 def test_config3_shear_layer_reduced(B, O, synth):
     c = synth.config3(nx=96, ny=128, nsteps=60)
+    q, w, st = run_gpu(B, c)
+    qo, wo, _ = run_oracle(O, c)
+    assert st["n_failed"] == 0
+    assert rel_l1(q, qo) <= 1e-8, rel_l1(q, qo)
+    assert rel_l1(w[:5], wo[:5]) <= 1e-8
+
+
+def test_config3_shear_layer_full_size(B, O, synth):
+    """BASELINE.json configs[2] as stated: 512 x 512, 200 steps, whole grid against the oracle (about a minute of
+    oracle time on 16 cores)."""
+    c = synth.config3()
+    assert c["prims"].shape[1:] == (1, 512, 512) and c["nsteps"] == 200
     q, w, st = run_gpu(B, c)
     qo, wo, _ = run_oracle(O, c)
     assert st["n_failed"] == 0
