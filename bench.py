@@ -112,6 +112,12 @@ def make_workload(name, synth):
         return synth.config4()
     if name == "cfg5_small":
         return synth.config5(n=64)
+    if name == "bw17":              # the paper's profile-table workload: 1-D Brio-Wu, nx = 2^17, sigma = 1e4
+        return synth.brio_wu_single(nx=2 ** 17, sigma=1e4)
+    if name == "khi":               # the paper's Fig 8 workload: 512 x 1024 KHI, single fluid
+        return synth.khi_paper(model=0)
+    if name == "khi2f":             # ... two-fluid
+        return synth.khi_paper(model=1)
     raise SystemExit(f"unknown workload {name}")
 
 

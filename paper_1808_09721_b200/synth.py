@@ -114,6 +114,88 @@ def config5(n=256, nsteps=20):
     return dict(name="cfg5_blast", params=params, prims=w, rho_charge=None, nsteps=nsteps, tol=1e-8)
 
 
+# ---------------------------------------------------------------------------------------------------
+# The paper's own set-ups: initial data as printed in PAPER.md section 4, used as
+# second / third workloads.  What the paper leaves open is fixed here and listed in DESIGN.md section 12.
+# ---------------------------------------------------------------------------------------------------
+def brio_wu_single(nx=200, sigma=1e4, t_end=0.4, cfl=0.4, integrator="ssp2"):
+    """Single-fluid resistive Brio-Wu tube, eq (13) PAPER.md L268 (set-up of Palenzuela et al. 2009): Gamma = 2,
+    (rho, p, B_y) = (1, 1, 0.5) | (0.125, 0.1, -0.5) on x in [0, 1], v = 0, E = 0, B_x = B_z = 0 (not printed: G14).
+    Fig 1 uses nx = 200, T = 0.4 (L287); the profile table nx = 2^17, sigma = 1e4 (L402)."""
+    x = cell_centres(nx, 0.0, 1.0)
+    left = x < 0.5
+    w = np.zeros((11, 1, 1, nx))
+    w[0, 0, 0] = np.where(left, 1.0, 0.125)
+    w[4, 0, 0] = np.where(left, 1.0, 0.1)
+    w[6, 0, 0] = np.where(left, 0.5, -0.5)
+    params = dict(model=RESISTIVE, nx=nx, ny=1, nz=1, ng=4, xlim=(0.0, 1.0), ylim=(0.0, 1.0), zlim=(0.0, 1.0),
+                  bc=(BC_OUTFLOW,) * 3, gamma=2.0, sigma=sigma, kappa=1.0, cfl=cfl, integrator=integrator)
+    nsteps = int(round(t_end / (cfl / nx)))
+    return dict(name="brio_wu_single", params=params, prims=w, rho_charge=None, nsteps=nsteps, tol=1e-9)
+
+
+def brio_wu_two_fluid(nx=400, mu_p=1e3, mu_e=-1e3, eta=1e-3, t_end=0.4, cfl=0.4, integrator="ssp2"):
+    """Two-fluid Brio-Wu tube, eq (14) PAPER.md L275 (initial data of Amano 2016):
+    (rho, p, B_x, B_y) = (1, 1, 0.5, 1) | (0.125, 0.1, 0.5, -1) on x in [0, 1], both species at rest, E = 0.
+    Fig 2 (L291): pair plasma mu_p = -mu_e = 1e3, and mu_p = 1e3, mu_e = -1e5, up to 1600 cells, T = 0.4.
+    Species split (not printed): charge neutral (sum_s mu_s rho_s = 0) and equal number density and temperature,
+    so rho_s = rho |mu_other| / (|mu_e| + |mu_p|) and p_e = p_p = p/2.  Gamma = 2 as in the single-fluid tube;
+    eta = 1e-3 (the paper gives none for this test)."""
+    x = cell_centres(nx, 0.0, 1.0)
+    left = x < 0.5
+    rho = np.where(left, 1.0, 0.125)
+    pr = np.where(left, 1.0, 0.1)
+    ae, ap = abs(mu_e), abs(mu_p)
+    w = np.zeros((16, 1, 1, nx))
+    w[0, 0, 0] = rho * ap / (ae + ap)
+    w[5, 0, 0] = rho * ae / (ae + ap)
+    w[4, 0, 0] = 0.5 * pr
+    w[9, 0, 0] = 0.5 * pr
+    w[10, 0, 0] = 0.5
+    w[11, 0, 0] = np.where(left, 1.0, -1.0)
+    params = dict(model=TWO_FLUID, nx=nx, ny=1, nz=1, ng=4, xlim=(0.0, 1.0), ylim=(0.0, 1.0), zlim=(0.0, 1.0),
+                  bc=(BC_OUTFLOW,) * 3, gamma=2.0, eta=eta, mu_e=mu_e, mu_p=mu_p, kappa=1.0, cfl=cfl, integrator=integrator)
+    nsteps = int(round(t_end / (cfl / nx)))
+    return dict(name="brio_wu_two_fluid", params=params, prims=w, rho_charge=None, nsteps=nsteps, tol=1e-8)
+
+
+def khi_paper(model=RESISTIVE, nx=512, ny=1024, nsteps=None, cfl=0.4, integrator="ssp2"):
+    """Double-shear-layer Kelvin-Helmholtz set-up, eq (18)-(20) PAPER.md L336-352 (adapted from Mignone et al. 2009):
+    x in [-0.5, 0.5], y in [-1, 1]; v_shear = 0.5, a = 0.01, (rho0, rho1) = (0.55, 0.45), A0 = 0.1, l = 0.1, p = 1,
+    Gamma = 4/3, B_z = 0.1, sigma = 10, mu_p = -mu_e = 100; 512 x 1024 cells, T = 6 (L350-354).
+    Not printed: boundary conditions (periodic in x and y here: the double layer is periodic in y), E (-v x B),
+    the two-fluid species split (rho_s = rho/2, p_s = p/2, v_s = v) and its resistivity (eta = 1/sigma)."""
+    vs, a, rho0, rho1, A0, ell = 0.5, 0.01, 0.55, 0.45, 0.1, 0.1
+    x = cell_centres(nx, -0.5, 0.5)[None, :]
+    y = cell_centres(ny, -1.0, 1.0)[:, None]
+    up = y > 0.0
+    ys = np.where(up, y - 0.5, y + 0.5)
+    sgn = np.where(up, 1.0, -1.0)
+    vx = sgn * vs * np.tanh(ys / a) + 0.0 * x
+    vy = sgn * A0 * vs * np.sin(2.0 * np.pi * x) * np.exp(-ys ** 2 / ell ** 2)
+    rho = rho0 + sgn * rho1 * np.tanh(ys / a) + 0.0 * x
+    v = np.zeros((3, 1, ny, nx)); v[0, 0] = vx; v[1, 0] = vy
+    B = np.zeros((3, 1, ny, nx)); B[2] = 0.1
+    E = _minus_v_cross_B(v, B)
+    common = dict(nx=nx, ny=ny, nz=1, ng=4, xlim=(-0.5, 0.5), ylim=(-1.0, 1.0), zlim=(0.0, 1.0),
+                  bc=(BC_PERIODIC, BC_PERIODIC, BC_PERIODIC), gamma=4.0 / 3.0, kappa=1.0, cfl=cfl, integrator=integrator)
+    if model == RESISTIVE:
+        w = np.zeros((11, 1, ny, nx))
+        w[0, 0] = rho; w[1:4] = v; w[4] = 1.0; w[5:8] = B; w[8:11] = E
+        params = dict(model=RESISTIVE, sigma=10.0, **common)
+    else:
+        w = np.zeros((16, 1, ny, nx))
+        for sp in range(2):
+            w[5 * sp, 0] = 0.5 * rho; w[5 * sp + 1:5 * sp + 4] = v; w[5 * sp + 4] = 0.5
+        w[10:13] = B; w[13:16] = E
+        params = dict(model=TWO_FLUID, eta=0.1, mu_e=-100.0, mu_p=100.0, **common)
+    dt = cfl / (nx / 1.0 + ny / 2.0)
+    if nsteps is None:
+        nsteps = int(round(6.0 / dt))
+    return dict(name="khi_paper_" + ("resistive" if model == RESISTIVE else "two_fluid"), params=params, prims=w,
+                rho_charge=None, nsteps=nsteps, tol=1e-8)
+
+
 def random_resistive_prims(n, seed, vmax=0.99, with_E=True):
     """Random admissible resistive primitive states (round-trip pins, kernel unit tests)."""
     rng = np.random.default_rng(seed)

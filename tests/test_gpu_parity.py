@@ -391,3 +391,27 @@ def test_ssp3_332_parity(B, O, synth, case, monkeypatch):
 def test_bad_integrator_is_rejected(B):
     with pytest.raises(B.RmhdError):
         B.Rmhd(model=0, nx=8, integrator=7)
+
+
+# ------------------------------------------------------------------------------------------
+# the paper's own set-ups (section 4), both integrators
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("integrator", ["ssp2", "ssp3"])
+@pytest.mark.parametrize("case", ["brio_wu_single_fig1", "brio_wu_pair", "brio_wu_electron_proton", "khi_resistive", "khi_two_fluid"])
+def test_paper_setups_parity(B, O, synth, case, integrator):
+    if case == "brio_wu_single_fig1":        # Fig 1: nx = 200, T = 0.4, sigma = 1e3
+        c = synth.brio_wu_single(nx=200, sigma=1e3, integrator=integrator); tol = 1e-9
+    elif case == "brio_wu_pair":             # Fig 2 left: mu_p = -mu_e = 1e3
+        c = synth.brio_wu_two_fluid(nx=200, mu_p=1e3, mu_e=-1e3, integrator=integrator); tol = 1e-8
+    elif case == "brio_wu_electron_proton":  # Fig 2 right: mu_p = 1e3, mu_e = -1e5
+        c = synth.brio_wu_two_fluid(nx=160, mu_p=1e3, mu_e=-1e5, integrator=integrator); tol = 1e-8
+    elif case == "khi_resistive":            # eq (18)-(20), reduced grid, 120 steps
+        c = synth.khi_paper(model=0, nx=64, ny=128, nsteps=120, integrator=integrator); tol = 1e-8
+    else:
+        c = synth.khi_paper(model=1, nx=48, ny=96, nsteps=60, integrator=integrator); tol = 1e-8
+    q, w, st = run_gpu(B, c)
+    qo, wo, sto = run_oracle(O, c)
+    assert st["n_failed"] == 0 and sto["n_failed"] == 0
+    assert rel_l1(q, qo) <= tol, rel_l1(q, qo)
+    nh = 5 if c["params"]["model"] == 0 else 10
+    assert rel_l1(w[:nh], wo[:nh]) <= 10 * tol
