@@ -16,10 +16,18 @@
 
 namespace rmhd {
 
-constexpr int HM_THREADS = 2 * FF_MAIN;
+// geometry of the two-role kernel: TX = 32 columns x TYP rows per CTA (TYP = 4: two CTAs per SM; TYP = 8: one CTA
+// of 16 warps per SM with half the y-halo and extra-face overhead per cell)
+template <int TYP> struct HMGeom {
+  static constexpr int NF = FSet<0>::NF, NC = R_NC, NHV = FSet<0>::NHV;
+  static constexpr int TY = TYP, MAIN = FF_TX * TYP, THREADS = 2 * MAIN, YR = TYP + 4;
+  static constexpr int GX = NF * TY * FF_XW, GY = NF * YR * FF_TX, FY = NC * (TY + 1) * FF_TX, FX = NC * TY, RING = 4 * NHV * MAIN;
+  static constexpr size_t bytes(bool has_z) { return sizeof(double) * (GX + GY + FY + FX + (has_z ? RING : 0)); }
+};
+constexpr int HM_THREADS = HMGeom<4>::THREADS;
 
 // CTA-wide barrier reached from role-specific code paths (every thread executes the same number of them)
-RMHD_DEV void hm_barrier() { asm volatile("bar.sync 1, %0;" ::"n"(HM_THREADS) : "memory"); }
+template <int NT> RMHD_DEV void hm_barrier() { asm volatile("bar.sync 1, %0;" ::"n"(NT) : "memory"); }
 
 // split-phase CTA barrier (mbarrier): arrive when the own shared-memory reads/writes of a phase are done, wait
 // only where the others' results are needed; independent work placed in between hides the skew between warps
@@ -76,18 +84,18 @@ __host__ __device__ constexpr int hm_mrow(int m) { return m < 6 ? 5 + m : (m == 
 #define RMHD_HM_GH 6     // reconstructions in flight per batch, role H (12 per face)
 #endif
 
-template <bool HAS_Z, bool COMB = false>
-__global__ void __launch_bounds__(HM_THREADS, 2)
+template <bool HAS_Z, bool COMB = false, int TYP = 4>
+__global__ void __launch_bounds__(HMGeom<TYP>::THREADS, TYP == 4 ? 2 : 1)
 k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int nx, int ny, int nz, int bcx, int bcy, int bcz,
           double hidx, double hidy, double hidz, int seg_len, DevPar P, FluxComb cb) {
   using FS = FSet<0>;
-  using SM = FFSmem<0>;
+  using SM = HMGeom<TYP>;
   constexpr int NC = R_NC, NH = R_NH, NF = FS::NF, NHV = FS::NHV, NM = 8;
-  constexpr int TX = FF_TX, TY = FF_TY, XW = FF_XW, YR = FF_YR;
+  constexpr int TX = FF_TX, TY = TYP, XW = FF_XW, YR = SM::YR, MAIN = SM::MAIN, NT = SM::THREADS;
   constexpr int FSX = TY * XW, FSY = YR * TX;       // field strides of gX, gY
   extern __shared__ double sm[];
   __shared__ unsigned long long bar2;                // "P2 done" (fY, fX written; gX, gY no longer read)
-  if (threadIdx.x == 0) mbar_init(&bar2, HM_THREADS);
+  if (threadIdx.x == 0) mbar_init(&bar2, NT);
   __syncthreads();
   unsigned ph2 = 0;
   double* gX = sm;
@@ -97,14 +105,14 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
   const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
   const bool roleH = wrp < TY;
   const int ty = wrp & (TY - 1);
-  double* ring = fX + SM::FX + (tid & (FF_MAIN - 1));   // role H only
+  double* ring = fX + SM::FX + (tid & (MAIN - 1));   // role H only
   const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
   const int i = i0 + lane, j = j0 + ty;
   const bool inside = i < nx && j < ny;
   const int im = bc_map(i, nx, bcx), jm = bc_map(j, ny, bcy);
-  const int hrow = ty < 2 ? ty : ty + 4;              // gY row of the y-halo cell of this M thread
+  const int hrow = ty < 2 ? ty : ty + TY;             // gY row of the y-halo cell of this M thread (M warps 0-3 only)
   const int jh = bc_map(j0 + hrow - 2, ny, bcy);
-  const int xh_row = (lane >> 2) & 3, xh_col = (lane & 3) < 2 ? (lane & 3) : (lane & 3) + 32;
+  const int xh_row = (lane >> 2) & (TY - 1), xh_col = (lane & 3) < 2 ? (lane & 3) : (lane & 3) + 32;
   const int ixh = bc_map(i0 + xh_col - 2, nx, bcx), jxh = bc_map(j0 + xh_row, ny, bcy);
   // 32-bit element offsets inside a row (N < 2^31, checked by rmhd_create): one IMAD.WIDE per access
   const unsigned pstride = (unsigned)nx * ny;
@@ -136,7 +144,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
   for (int v = 0; v < NHV; ++v) pend[v] = 0.0;
 #pragma unroll
   for (int v = 0; v < NM; ++v) Gprev[v] = 0.0;
-  int s_old = 0, s_new = 2 * NHV * FF_MAIN;
+  int s_old = 0, s_new = 2 * NHV * MAIN;
 
   const int cbeg = HAS_Z ? k0 - 2 : 2, cend = HAS_Z ? k1 + 1 : 2;
 #pragma unroll 1
@@ -171,7 +179,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
             gY[((NHV + h) * YR + ty + 2) * TX + lane] = fh[h] - q_[FS::hv(h)];
           }
         }
-        hm_barrier();
+        hm_barrier<NT>();
         // left x-face (t = 0) and bottom y-face (t = 1) of the own cell: ONE copy of the reconstruction code
 #pragma unroll 1
         for (int t = 0; t < 2; ++t) {
@@ -215,8 +223,8 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
 #pragma unroll
             for (int g = 0; g < G; ++g) {
               const int f = f0 + g;
-              const double u2 = ring[s_old + f * FF_MAIN];
-              b[g] = ring[s_new + f * FF_MAIN];
+              const double u2 = ring[s_old + f * MAIN];
+              b[g] = ring[s_new + f * MAIN];
               if (f < NHV) { a[g] = u2; cc[g] = u0[f]; } else { a[g] = u0[f]; cc[g] = u2; }
             }
             weno3_batch<G, true>(a, b, cc, o + f0);
@@ -230,7 +238,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
           }
         }
 #pragma unroll
-        for (int f = 0; f < 2 * NHV; ++f) ring[s_old + f * FF_MAIN] = u0[f];
+        for (int f = 0; f < 2 * NHV; ++f) ring[s_old + f * MAIN] = u0[f];
         { const int t = s_old; s_old = s_new; s_new = t; }
       }
       if (do_xy) {
@@ -254,8 +262,8 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
         if (inside) prefetch_rows<COMB, NM>(cb, N, pk + (unsigned)j * nx + i, [](int m) { return hm_mrow(m); });
         if (HAS_Z && c < cend) {
           const unsigned pn = (unsigned)(k + 1) * pstride;
-          prefetch_cell(pn + col_yh);
-          if (wrp == 2 * TY - 1 && lane < 16) prefetch_cell(pn + col_xh);
+          if (TY == 4 || ty < 4) prefetch_cell(pn + col_yh);
+          if (wrp == 2 * TY - 1 && lane < 4 * TY) prefetch_cell(pn + col_xh);
         }
       }
       {
@@ -296,12 +304,14 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
         {
           double q_[NC], w_[NH], g[NF];
           Com<0> cm;
-          load_cell(pk + col_yh, q_, w_);
-          cell_common(q_, w_, P, cm);
-          cell_fields<0, 1>(q_, w_, cm, P, g);
+          if (TY == 4 || ty < 4) {                   // the 4 y-halo rows: M warps 0-3
+            load_cell(pk + col_yh, q_, w_);
+            cell_common(q_, w_, P, cm);
+            cell_fields<0, 1>(q_, w_, cm, P, g);
 #pragma unroll
-          for (int f = 0; f < NF; ++f) gY[(f * YR + hrow) * TX + lane] = g[f];
-          if (wrp == 2 * TY - 1 && lane < 16) {
+            for (int f = 0; f < NF; ++f) gY[(f * YR + hrow) * TX + lane] = g[f];
+          }
+          if (wrp == 2 * TY - 1 && lane < 4 * TY) {
             load_cell(pk + col_xh, q_, w_);
             cell_common(q_, w_, P, cm);
             cell_fields<0, 0>(q_, w_, cm, P, g);
@@ -309,13 +319,14 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
             for (int f = 0; f < NF; ++f) gX[(f * TY + xh_row) * XW + xh_col] = g[f];
           }
         }
-        hm_barrier();
-        // t = 0: left x-face, t = 1: bottom y-face of the own cell; t = 2 (warps TY, TY+1 only): the 5th row of
+        hm_barrier<NT>();
+        // t = 0: left x-face, t = 1: bottom y-face of the own cell; t = 2 (two M warps only): the last row of
         // y-faces / the 33rd x-face of row `lane` (lanes >= TY reconstruct in-bounds garbage that is not stored)
-        const int ntask = wrp < TY + 2 ? 3 : 2;
+        constexpr int XB = TY == 4 ? 0 : 4;          // first of the 4 M warps that take the extra faces (TY = 8: those without a y-halo row)
+        const int ntask = (wrp == TY + XB || wrp == TY + XB + 1) ? 3 : 2;
 #pragma unroll 1
         for (int t = 0; t < ntask; ++t) {
-          const bool ydir = t == 1 || (t == 2 && wrp == TY);
+          const bool ydir = t == 1 || (t == 2 && wrp == TY + XB);
           const double* p = t == 0 ? gX + ty * XW + lane : (t == 1 ? gY + ty * TX + lane : (ydir ? gY + TY * TX + lane : gX + lane * XW + TX));
           double o[NM], G[NM];
           face_recon_range<2 * NHV, NM, NM>(p, ydir ? FSY : FSX, ydir ? TX : 1, o);
@@ -337,8 +348,8 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
             for (int v = 0; v < NM; ++v) fX[hm_mrow(v) * TY + lane] = G[v];
           }
         }
-        if (wrp >= TY + 2) {       // the same two extra face sets of the hydro rows (12 fields), taken off role H
-          const bool ydir = wrp == TY + 2;
+        if (wrp == TY + XB + 2 || wrp == TY + XB + 3) {   // the same two extra face sets of the hydro rows (12 fields), taken off role H
+          const bool ydir = wrp == TY + XB + 2;
           double o[2 * NHV];
           face_recon_range<0, 2 * NHV, RMHD_HM_GH>(ydir ? gY + TY * TX + lane : gX + (lane & (TY - 1)) * XW + TX, ydir ? FSY : FSX, ydir ? TX : 1, o);
           if (ydir) {

@@ -40,6 +40,7 @@ struct rmhd_ctx {
   bool profiling;
   bool fused_flux;   // one-pass L(q) over all axes (flux_fused.cuh) when nx, ny > 1; RMHD_FLUX=split forces the per-axis kernels
   bool fuse_combine; // eq (11) in the epilogue of the F2 flux launch (fused path only); RMHD_COMBINE=split keeps k_final
+  int hm_ty;         // tile rows of the two-role flux kernel: 8 (one 16-warp CTA per SM; default when ny >= 8) or 4 (two CTAs); RMHD_HM_TY
   bool one_role;     // RMHD_FLUX=fused1: resistive model through the one-thread-per-column kernel (flux_fused.cuh) instead of flux_hm.cuh
   int sm_count;
   std::vector<EvRec> pending;
@@ -151,23 +152,26 @@ int launch_flux_axis(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODEL
   return RMHD_OK;
 }
 
-// all present axes in one pass (flux_fused.cuh); needs nx > 1 and ny > 1
-template <int MODEL, bool HAS_Z, bool COMB>
+// all present axes in one pass (flux_fused.cuh, flux_hm.cuh); needs nx > 1 and ny > 1.  TYP: tile rows of the two-role kernel
+template <int MODEL, bool HAS_Z, bool COMB, int TYP>
 int launch_flux_fused(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODEL>& wr, double* L, const FluxComb& cb) {
   static bool attr_set[8] = {false, false, false, false, false, false, false, false};
   const int nx = c->n[0], ny = c->n[1], nz = c->n[2];
-  const size_t smem = FFSmem<MODEL>::bytes(HAS_Z);
+  bool two_role = false;
+  if constexpr (MODEL == 0) two_role = !c->one_role;
+  const int ty = two_role ? TYP : FF_TY;
+  const size_t smem = two_role ? HMGeom<TYP>::bytes(HAS_Z) : FFSmem<MODEL>::bytes(HAS_Z);
   if (!attr_set[c->device & 7]) {
-    CK(c, cudaFuncSetAttribute(k_flux_fused<MODEL, HAS_Z, COMB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    if constexpr (MODEL == 0) CK(c, cudaFuncSetAttribute(k_flux_hm<HAS_Z, COMB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CK(c, cudaFuncSetAttribute(k_flux_fused<MODEL, HAS_Z, COMB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFSmem<MODEL>::bytes(HAS_Z)));
+    if constexpr (MODEL == 0) CK(c, cudaFuncSetAttribute(k_flux_hm<HAS_Z, COMB, TYP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)HMGeom<TYP>::bytes(HAS_Z)));
     attr_set[c->device & 7] = true;
   }
-  const int gx = (nx + FF_TX - 1) / FF_TX, gy = (ny + FF_TY - 1) / FF_TY;
+  const int gx = (nx + FF_TX - 1) / FF_TX, gy = (ny + ty - 1) / ty;
   int nseg = 1, seg_len = 1;
   if (HAS_Z) {
     // z segments: pick the count (segments of >= 16 planes) that wastes least, counting the partially filled
-    // last wave of resident CTAs (2 per SM) and the 4 feed-only prologue planes of every segment
-    const long long tiles = (long long)gx * gy, slots = 2LL * c->sm_count;
+    // last wave of resident CTAs and the 4 feed-only prologue planes of every segment
+    const long long tiles = (long long)gx * gy, slots = (two_role && TYP == 8 ? 1LL : 2LL) * c->sm_count;
     double best = 1e300;
     for (int s = 1; s <= (nz + 15) / 16 && s <= 64; ++s) {
       const int len = (nz + s - 1) / s, cnt = (nz + len - 1) / len;
@@ -178,12 +182,10 @@ int launch_flux_fused(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODE
   }
   dim3 grid(gx, gy, nseg);
   Timed t(c, KC_FLUX);
-  bool two_role = false;
-  if constexpr (MODEL == 0) two_role = !c->one_role;
   if constexpr (MODEL == 0) {
     if (two_role)
-      k_flux_hm<HAS_Z, COMB><<<grid, HM_THREADS, smem, c->stream>>>(qr, wr, L, c->N, nx, ny, nz, c->p.bc[0], c->p.bc[1], c->p.bc[2],
-                                                                  0.5 / c->dx[0], 0.5 / c->dx[1], 0.5 / c->dx[2], seg_len, c->P, cb);
+      k_flux_hm<HAS_Z, COMB, TYP><<<grid, HMGeom<TYP>::THREADS, smem, c->stream>>>(qr, wr, L, c->N, nx, ny, nz, c->p.bc[0], c->p.bc[1], c->p.bc[2],
+                                                                                 0.5 / c->dx[0], 0.5 / c->dx[1], 0.5 / c->dx[2], seg_len, c->P, cb);
   }
   if (!two_role)
     k_flux_fused<MODEL, HAS_Z, COMB><<<grid, FF_THREADS, smem, c->stream>>>(qr, wr, L, c->N, nx, ny, nz, c->p.bc[0], c->p.bc[1], c->p.bc[2],
@@ -191,9 +193,12 @@ int launch_flux_fused(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODE
   CK(c, cudaGetLastError());
   return RMHD_OK;
 }
+template <int MODEL, bool HAS_Z, bool COMB>
+int launch_flux_fused(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODEL>& wr, double* L, const FluxComb& cb) {
+  if (MODEL == 0 && c->hm_ty == 8) return launch_flux_fused<MODEL, HAS_Z, COMB, 8>(c, qr, wr, L, cb);
+  return launch_flux_fused<MODEL, HAS_Z, COMB, 4>(c, qr, wr, L, cb);
+}
 
-// L(q) with the conserved rows taken from `qa` except the rows listed in src rows, which come
-// from `qb` when mix != 0 (stage 1 only rewrites the rows that have a source).
 inline bool uses_fused_flux(const rmhd_ctx* c) { return c->fused_flux && c->n[0] > 1 && c->n[1] > 1; }
 
 // `cb` (fused path only): store the eq-(11) update of q instead of L (a5 fused into F2)
@@ -360,6 +365,7 @@ int rmhd_create(const rmhd_params* p, rmhd_ctx** out) {
   { const char* e = getenv("RMHD_FLUX"); c->fused_flux = !(e && strcmp(e, "split") == 0); }
   { const char* e = getenv("RMHD_FLUX"); c->one_role = e && strcmp(e, "fused1") == 0; }
   { const char* e = getenv("RMHD_COMBINE"); c->fuse_combine = !(e && strcmp(e, "split") == 0); }
+  { const char* e = getenv("RMHD_HM_TY"); c->hm_ty = e ? (atoi(e) == 8 ? 8 : 4) : (p->ny >= 8 ? 8 : 4); }
   c->sm_count = 148;
   for (int i = 0; i < KC_N; ++i) { c->ms[i] = 0.0; c->launches[i] = 0; }
   c->q = c->w = c->qs = c->L1 = c->L2 = c->Ps1 = c->Ps2 = c->A = nullptr; c->d_stats = nullptr; c->h_stats = nullptr;
