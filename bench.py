@@ -230,18 +230,21 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     # ---- device-resident timing -------------------------------------------------------------
+    # K steps through one rmhd_step(ctx, K) call (one statistics read and stream sync at its end), CUDA events on the
+    # library's stream around it; a second, instrumented pass of K steps (an event pair around every launch) gives the
+    # per-kernel times the roofline object uses, so that instrumentation does not sit inside the timed region.
     for _ in range(args.warmup):
         sim.step(1)
-    B.rmhd_set_profiling(sim.ctx, True)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     with ClockSampler(local) as clk:
         ev0.record()
-        for _ in range(args.steps):
-            sim.step(1)
+        sim.step(args.steps)
         ev1.record()
         barrier()
     ms_total = ev0.elapsed_time(ev1)
+    B.rmhd_set_profiling(sim.ctx, True)
+    sim.step(args.steps)
     kt = B.rmhd_get_kernel_times(sim.ctx)
     stats = sim.stats()
     B.rmhd_set_profiling(sim.ctx, False)
