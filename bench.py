@@ -186,6 +186,21 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+# ---- replicas-only aggregation --------------------------------------------
+def whole_job_rate(ms_local, units_local, dist, device):
+    """Whole-job throughput over all ranks: units of every rank summed, divided by the slowest rank's device time.
+    No data-path collective exists (each rank steps its own replica); these two reductions are the only exchange.
+    Returns (units per second, max ms).  `dist` is torch.distributed or None (one process)."""
+    import torch
+    t = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    u = torch.tensor([float(units_local)], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    ms = float(t.item())
+    return float(u.item()) / (ms * 1e-3), ms
+
+
 # ---- our arm ----------------------------------------------------------------------------------
 def stage_flops(hist):
     """Algorithmic flops of one resistive implicit-stage launch from the logged iteration histogram.
@@ -248,11 +263,7 @@ def run_ours(args):
     kt = B.rmhd_get_kernel_times(sim.ctx)
     stats = sim.stats()
     B.rmhd_set_profiling(sim.ctx, False)
-    t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total = float(t.item())
-    value = world * ncell * args.steps / (ms_total * 1e-3)
+    value, ms_total = whole_job_rate(ms_total, ncell * args.steps, dist, dev)
 
     # ---- roofline of the dominant kernel class -------------------------------------------------
     naxes = sum(1 for n in (nx, ny, nz) if n > 1)
@@ -313,10 +324,8 @@ def run_ours(args):
             B.rmhd_get_state(sim.ctx, cons_h, None)        # D2H of the step's result
         ev1.record()
         barrier()
-        t = torch.tensor([ev0.elapsed_time(ev1)], dtype=torch.float64, device=dev)
-        if dist is not None:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * ncell * e_steps / (float(t.item()) * 1e-3), "unit": UNIT,
+        e_rate, _ = whole_job_rate(ev0.elapsed_time(ev1), ncell * e_steps, dist, dev)
+        e2e = {"value": e_rate, "unit": UNIT,
                "h2d_bytes_per_step": nc * ncell * 8, "d2h_bytes_per_step": nc * ncell * 8,
                "steps": e_steps, "call": "rmhd_set_cons(host cons) + rmhd_step(1) + rmhd_get_state(host cons), pinned host buffers"}
         del cons_h
