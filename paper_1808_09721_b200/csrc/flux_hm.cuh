@@ -84,7 +84,11 @@ __host__ __device__ constexpr int hm_mrow(int m) { return m < 6 ? 5 + m : (m == 
 #define RMHD_HM_GH 6     // reconstructions in flight per batch, role H (12 per face)
 #endif
 
-template <bool HAS_Z, bool COMB = false, int TYP = 4>
+// HAS_Y = false (2-D grids): the tile's TY rows are TY consecutive 32-cell segments of one x line, there is no y work in
+// the plane, and the marching axis ("z" below) is the grid's y axis: ZDIR = 1 selects the y components of the flux
+// vectors; the host passes ny = 1, nz = the grid's ny, bcz = its y boundary condition, hidz = 1/(2 dy).  A 2-D grid
+// then runs the same plane pipeline as a 3-D one instead of one isolated plane per CTA.
+template <bool HAS_Z, bool COMB = false, int TYP = 4, bool HAS_Y = true, int ZDIR = 2>
 __global__ void __launch_bounds__(HMGeom<TYP>::THREADS, TYP == 4 ? 2 : 1)
 k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int nx, int ny, int nz, int bcx, int bcy, int bcz,
           double hidx, double hidy, double hidz, int seg_len, DevPar P, FluxComb cb) {
@@ -106,14 +110,16 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
   const bool roleH = wrp < TY;
   const int ty = wrp & (TY - 1);
   double* ring = fX + SM::FX + (tid & (MAIN - 1));   // role H only
-  const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
-  const int i = i0 + lane, j = j0 + ty;
+  const int i0 = HAS_Y ? blockIdx.x * TX : blockIdx.x * (TX * TY) + ty * TX;   // first column of this thread's row
+  const int j0 = HAS_Y ? blockIdx.y * TY : 0;
+  const int i = i0 + lane, j = HAS_Y ? j0 + ty : 0;
   const bool inside = i < nx && j < ny;
   const int im = bc_map(i, nx, bcx), jm = bc_map(j, ny, bcy);
   const int hrow = ty < 2 ? ty : ty + TY;             // gY row of the y-halo cell of this M thread (M warps 0-3 only)
   const int jh = bc_map(j0 + hrow - 2, ny, bcy);
   const int xh_row = (lane >> 2) & (TY - 1), xh_col = (lane & 3) < 2 ? (lane & 3) : (lane & 3) + 32;
-  const int ixh = bc_map(i0 + xh_col - 2, nx, bcx), jxh = bc_map(j0 + xh_row, ny, bcy);
+  const int ixh = bc_map((HAS_Y ? i0 : (int)blockIdx.x * (TX * TY) + xh_row * TX) + xh_col - 2, nx, bcx);
+  const int jxh = HAS_Y ? bc_map(j0 + xh_row, ny, bcy) : 0;
   // 32-bit element offsets inside a row (N < 2^31, checked by rmhd_create): one IMAD.WIDE per access
   const unsigned pstride = (unsigned)nx * ny;
   const unsigned col_main = (unsigned)jm * nx + im, col_yh = (unsigned)jh * nx + im, col_xh = (unsigned)jxh * nx + ixh;
@@ -172,17 +178,19 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
             gX[(h * TY + ty) * XW + lane + 2] = fh[h] + q_[FS::hv(h)];
             gX[((NHV + h) * TY + ty) * XW + lane + 2] = fh[h] - q_[FS::hv(h)];
           }
-          cell_hflux<1>(q_, w_, cm, P, fh);
+          if (HAS_Y) {
+            cell_hflux<1>(q_, w_, cm, P, fh);
 #pragma unroll
-          for (int h = 0; h < NHV; ++h) {
-            gY[(h * YR + ty + 2) * TX + lane] = fh[h] + q_[FS::hv(h)];
-            gY[((NHV + h) * YR + ty + 2) * TX + lane] = fh[h] - q_[FS::hv(h)];
+            for (int h = 0; h < NHV; ++h) {
+              gY[(h * YR + ty + 2) * TX + lane] = fh[h] + q_[FS::hv(h)];
+              gY[((NHV + h) * YR + ty + 2) * TX + lane] = fh[h] - q_[FS::hv(h)];
+            }
           }
         }
         hm_barrier<NT>();
         // left x-face (t = 0) and bottom y-face (t = 1) of the own cell: ONE copy of the reconstruction code
 #pragma unroll 1
-        for (int t = 0; t < 2; ++t) {
+        for (int t = 0; t < (HAS_Y ? 2 : 1); ++t) {
           double o[2 * NHV];
           face_recon_range<0, 2 * NHV, RMHD_HM_GH>(t ? gY + ty * TX + lane : gX + ty * XW + lane, t ? FSY : FSX, t ? TX : 1, o);
           if (t == 0) {
@@ -210,7 +218,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
           Com<0> cm;
           load_cell((unsigned)bc_map(c, nz, bcz) * pstride + col_main, q_, w_);
           cell_common(q_, w_, P, cm);
-          cell_hflux<2>(q_, w_, cm, P, fh);
+          cell_hflux<ZDIR>(q_, w_, cm, P, fh);
 #pragma unroll
           for (int h = 0; h < NHV; ++h) { u0[h] = fh[h] + q_[FS::hv(h)]; u0[NHV + h] = fh[h] - q_[FS::hv(h)]; }
         }
@@ -244,7 +252,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
       if (do_xy) {
         mbar_wait(&bar2, ph2); ph2 ^= 1u;
 #pragma unroll
-        for (int h = 0; h < NHV; ++h) Lacc[h] = fma(-fY[(FS::hv(h) * (TY + 1) + ty + 1) * TX + lane], hidy, Lacc[h]);
+        for (int h = 0; h < NHV; ++h) if (HAS_Y) Lacc[h] = fma(-fY[(FS::hv(h) * (TY + 1) + ty + 1) * TX + lane], hidy, Lacc[h]);
         if (lane == 31) {
 #pragma unroll
           for (int h = 0; h < NHV; ++h) Lacc[h] = fma(-fX[FS::hv(h) * TY + ty], hidx, Lacc[h]);
@@ -262,7 +270,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
         if (inside) prefetch_rows<COMB, NM>(cb, N, pk + (unsigned)j * nx + i, [](int m) { return hm_mrow(m); });
         if (HAS_Z && c < cend) {
           const unsigned pn = (unsigned)(k + 1) * pstride;
-          if (TY == 4 || ty < 4) prefetch_cell(pn + col_yh);
+          if (HAS_Y && (TY == 4 || ty < 4)) prefetch_cell(pn + col_yh);
           if (wrp == 2 * TY - 1 && lane < 4 * TY) prefetch_cell(pn + col_xh);
         }
       }
@@ -276,16 +284,18 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
             mx_fields<0>(B, E, psi, phi, m);
 #pragma unroll
             for (int f = 0; f < NM; ++f) gX[((2 * NHV + f) * TY + ty) * XW + lane + 2] = m[f];
-            mx_fields<1>(B, E, psi, phi, m);
+            if (HAS_Y) {
+              mx_fields<1>(B, E, psi, phi, m);
 #pragma unroll
-            for (int f = 0; f < NM; ++f) gY[((2 * NHV + f) * YR + ty + 2) * TX + lane] = m[f];
+              for (int f = 0; f < NM; ++f) gY[((2 * NHV + f) * YR + ty + 2) * TX + lane] = m[f];
+            }
           }
           if (HAS_Z) {
-            mx_fields<2>(B, E, psi, phi, u2);
+            mx_fields<ZDIR>(B, E, psi, phi, u2);
             load_mx((unsigned)bc_map(c - 1, nz, bcz) * pstride + col_main, B, E, psi, phi);
-            mx_fields<2>(B, E, psi, phi, u1);
+            mx_fields<ZDIR>(B, E, psi, phi, u1);
             load_mx((unsigned)bc_map(c, nz, bcz) * pstride + col_main, B, E, psi, phi);
-            mx_fields<2>(B, E, psi, phi, u0);
+            mx_fields<ZDIR>(B, E, psi, phi, u0);
           }
         }
         if (HAS_Z && c >= k0) {
@@ -295,7 +305,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
           weno3_batch<NM, true>(a, u1, cc, o);
 #pragma unroll
           for (int g = 0; g < 4; ++g) { oo[g] = pend[g]; pend[g] = o[g]; oo[4 + g] = o[4 + g]; }
-          assemble_M<2>(oo, G);
+          assemble_M<ZDIR>(oo, G);
 #pragma unroll
           for (int v = 0; v < NM; ++v) { if (do_xy) Lacc[v] = (Gprev[v] - G[v]) * hidz; Gprev[v] = G[v]; }
         }
@@ -304,7 +314,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
         {
           double q_[NC], w_[NH], g[NF];
           Com<0> cm;
-          if (TY == 4 || ty < 4) {                   // the 4 y-halo rows: M warps 0-3
+          if (HAS_Y && (TY == 4 || ty < 4)) {        // the 4 y-halo rows: M warps 0-3
             load_cell(pk + col_yh, q_, w_);
             cell_common(q_, w_, P, cm);
             cell_fields<0, 1>(q_, w_, cm, P, g);
@@ -326,6 +336,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
         const int ntask = (wrp == TY + XB || wrp == TY + XB + 1) ? 3 : 2;
 #pragma unroll 1
         for (int t = 0; t < ntask; ++t) {
+          if (!HAS_Y && (t == 1 || (t == 2 && wrp == TY + XB))) continue;   // no y faces
           const bool ydir = t == 1 || (t == 2 && wrp == TY + XB);
           const double* p = t == 0 ? gX + ty * XW + lane : (t == 1 ? gY + ty * TX + lane : (ydir ? gY + TY * TX + lane : gX + lane * XW + TX));
           double o[NM], G[NM];
@@ -348,7 +359,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
             for (int v = 0; v < NM; ++v) fX[hm_mrow(v) * TY + lane] = G[v];
           }
         }
-        if (wrp == TY + XB + 2 || wrp == TY + XB + 3) {   // the same two extra face sets of the hydro rows (12 fields), taken off role H
+        if ((HAS_Y && wrp == TY + XB + 2) || wrp == TY + XB + 3) {   // the same two extra face sets of the hydro rows (12 fields), taken off role H
           const bool ydir = wrp == TY + XB + 2;
           double o[2 * NHV];
           face_recon_range<0, 2 * NHV, RMHD_HM_GH>(ydir ? gY + TY * TX + lane : gX + (lane & (TY - 1)) * XW + TX, ydir ? FSY : FSX, ydir ? TX : 1, o);
@@ -363,7 +374,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
         mbar_arrive(&bar2);
         mbar_wait(&bar2, ph2); ph2 ^= 1u;
 #pragma unroll
-        for (int v = 0; v < NM; ++v) Lacc[v] = fma(-fY[(hm_mrow(v) * (TY + 1) + ty + 1) * TX + lane], hidy, Lacc[v]);
+        for (int v = 0; v < NM; ++v) if (HAS_Y) Lacc[v] = fma(-fY[(hm_mrow(v) * (TY + 1) + ty + 1) * TX + lane], hidy, Lacc[v]);
         if (lane == 31) {
 #pragma unroll
           for (int v = 0; v < NM; ++v) Lacc[v] = fma(-fX[hm_mrow(v) * TY + ty], hidx, Lacc[v]);

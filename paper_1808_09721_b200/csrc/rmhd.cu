@@ -41,6 +41,7 @@ struct rmhd_ctx {
   bool fused_flux;   // one-pass L(q) over all axes (flux_fused.cuh) when nx, ny > 1; RMHD_FLUX=split forces the per-axis kernels
   bool fuse_combine; // eq (11) in the epilogue of the F2 flux launch (fused path only); RMHD_COMBINE=split keeps k_final
   int hm_ty;         // tile rows of the two-role flux kernel: 8 (one 16-warp CTA per SM; default when ny >= 8) or 4 (two CTAs); RMHD_HM_TY
+  bool march2d;      // resistive 2-D grids through the marching two-role kernel (default); RMHD_FLUX2D=tile keeps one plane per CTA
   bool one_role;     // RMHD_FLUX=fused1: resistive model through the one-thread-per-column kernel (flux_fused.cuh) instead of flux_hm.cuh
   int sm_count;
   std::vector<EvRec> pending;
@@ -199,6 +200,39 @@ int launch_flux_fused(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODE
   return launch_flux_fused<MODEL, HAS_Z, COMB, 4>(c, qr, wr, L, cb);
 }
 
+// resistive 2-D grids: the two-role kernel with the tile rows laid along x and the grid's y axis as the marching axis
+// (flux_hm.cuh, HAS_Y = false, ZDIR = 1)
+template <bool COMB>
+int launch_flux_march2d(rmhd_ctx* c, const ConsRows<0>& qr, const HydRows<0>& wr, double* L, const FluxComb& cb) {
+  static bool attr_set[8] = {false, false, false, false, false, false, false, false};
+  constexpr int TYP = 8;
+  const int nx = c->n[0], ny = c->n[1];
+  const size_t smem = HMGeom<TYP>::bytes(true);
+  if (!attr_set[c->device & 7]) {
+    CK(c, cudaFuncSetAttribute(k_flux_hm<true, COMB, TYP, false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr_set[c->device & 7] = true;
+  }
+  const int gx = (nx + FF_TX * TYP - 1) / (FF_TX * TYP);
+  // segments along y: fill the SMs (one CTA each), at least 4 planes per segment, then the same waste measure as in 3-D
+  int nseg = 1, seg_len = ny;
+  {
+    const long long slots = c->sm_count;
+    double best = 1e300;
+    for (int s = 1; s <= (ny + 3) / 4 && s <= 4096; ++s) {
+      const int len = (ny + s - 1) / s, cnt = (ny + len - 1) / len;
+      const long long ctas = (long long)gx * cnt, waves = (ctas + slots - 1) / slots;
+      const double cost = (double)waves * slots / (double)ctas * (1.0 + 1.5 / len);   // 4 feed-only planes ~ 1.5 full ones
+      if (cost < best - 1e-9) { best = cost; nseg = cnt; seg_len = len; }
+    }
+  }
+  dim3 grid(gx, 1, nseg);
+  Timed t(c, KC_FLUX);
+  k_flux_hm<true, COMB, TYP, false, 1><<<grid, HMGeom<TYP>::THREADS, smem, c->stream>>>(
+      qr, wr, L, c->N, nx, 1, ny, c->p.bc[0], 0, c->p.bc[1], 0.5 / c->dx[0], 0.0, 0.5 / c->dx[1], seg_len, c->P, cb);
+  CK(c, cudaGetLastError());
+  return RMHD_OK;
+}
+
 inline bool uses_fused_flux(const rmhd_ctx* c) { return c->fused_flux && c->n[0] > 1 && c->n[1] > 1; }
 
 // `cb` (fused path only): store the eq-(11) update of q instead of L (a5 fused into F2)
@@ -211,6 +245,9 @@ int launch_flux(rmhd_ctx* c, const double* qa, const double* qb, bool mix, const
   for (int v = 0; v < NH; ++v) wr.r[v] = w + (size_t)v * c->N;
   if (uses_fused_flux(c)) {
     const FluxComb none = {nullptr, nullptr, 0.0};
+    if constexpr (MODEL == 0) {
+      if (c->n[2] == 1 && c->march2d && !c->one_role) return cb ? launch_flux_march2d<true>(c, qr, wr, L, *cb) : launch_flux_march2d<false>(c, qr, wr, L, none);
+    }
     if (cb) return c->n[2] > 1 ? launch_flux_fused<MODEL, true, true>(c, qr, wr, L, *cb) : launch_flux_fused<MODEL, false, true>(c, qr, wr, L, *cb);
     return c->n[2] > 1 ? launch_flux_fused<MODEL, true, false>(c, qr, wr, L, none) : launch_flux_fused<MODEL, false, false>(c, qr, wr, L, none);
   }
@@ -365,6 +402,7 @@ int rmhd_create(const rmhd_params* p, rmhd_ctx** out) {
   { const char* e = getenv("RMHD_FLUX"); c->fused_flux = !(e && strcmp(e, "split") == 0); }
   { const char* e = getenv("RMHD_FLUX"); c->one_role = e && strcmp(e, "fused1") == 0; }
   { const char* e = getenv("RMHD_COMBINE"); c->fuse_combine = !(e && strcmp(e, "split") == 0); }
+  { const char* e = getenv("RMHD_FLUX2D"); c->march2d = !(e && strcmp(e, "tile") == 0); }
   { const char* e = getenv("RMHD_HM_TY"); c->hm_ty = e ? (atoi(e) == 8 ? 8 : 4) : (p->ny >= 8 ? 8 : 4); }
   c->sm_count = 148;
   for (int i = 0; i < KC_N; ++i) { c->ms[i] = 0.0; c->launches[i] = 0; }
