@@ -18,8 +18,8 @@ namespace rmhd {
 
 // geometry of the two-role kernel: TX = 32 columns x TYP rows per CTA (TYP = 4: two CTAs per SM; TYP = 8: one CTA
 // of 16 warps per SM with half the y-halo and extra-face overhead per cell)
-template <int TYP> struct HMGeom {
-  static constexpr int NF = FSet<0>::NF, NC = R_NC, NHV = FSet<0>::NHV;
+template <int TYP, int MODEL = 0> struct HMGeom {
+  static constexpr int NF = FSet<MODEL>::NF, NC = Dim<MODEL>::NC, NHV = FSet<MODEL>::NHV;
   static constexpr int TY = TYP, MAIN = FF_TX * TYP, THREADS = 2 * MAIN, YR = TYP + 4;
   static constexpr int GX = NF * TY * FF_XW, GY = NF * YR * FF_TX, FY = NC * (TY + 1) * FF_TX, FX = NC * TY, RING = 4 * NHV * MAIN;
   static constexpr size_t bytes(bool has_z) { return sizeof(double) * (GX + GY + FY + FX + (has_z ? RING : 0)); }
@@ -50,7 +50,7 @@ RMHD_DEV void mbar_wait(unsigned long long* bar, unsigned parity) {
 }
 
 // reconstructions of NREC consecutive fields starting at field F0 of one face (shared memory), G at a time
-template <int F0, int NREC, int G, int DONE = 0>
+template <int MODEL, int F0, int NREC, int G, int DONE = 0>
 RMHD_DEV void face_recon_range(const double* p, int fs, int st, double* o) {
   constexpr int B = NREC - DONE >= G ? G : NREC - DONE;
   double a[B], b[B], c[B];
@@ -58,11 +58,11 @@ RMHD_DEV void face_recon_range(const double* p, int fs, int st, double* o) {
   for (int g = 0; g < B; ++g) {
     const int f = F0 + DONE + g;
     const double* pf = p + f * fs;
-    if (field_is_plus<0>(f)) { a[g] = pf[0]; b[g] = pf[st]; c[g] = pf[2 * st]; }
+    if (field_is_plus<MODEL>(f)) { a[g] = pf[0]; b[g] = pf[st]; c[g] = pf[2 * st]; }
     else { a[g] = pf[3 * st]; b[g] = pf[2 * st]; c[g] = pf[st]; }
   }
   weno3_batch<B, true>(a, b, c, o + DONE);
-  if constexpr (DONE + B < NREC) face_recon_range<F0, NREC, G, DONE + B>(p, fs, st, o);
+  if constexpr (DONE + B < NREC) face_recon_range<MODEL, F0, NREC, G, DONE + B>(p, fs, st, o);
 }
 
 // G of the 8 Maxwell rows in the fixed order (Bx, By, Bz, Ex, Ey, Ez, psi, phi) from P1..P4, M1..M4 of axis K
@@ -78,7 +78,9 @@ RMHD_DEV void assemble_M(const double* p, double* G) {
   G[3 + K] = p[3] + p[7];
   G[6] = p[3] - p[7];
 }
-__host__ __device__ constexpr int hm_mrow(int m) { return m < 6 ? 5 + m : (m == 6 ? 12 : 13); }   // conserved row of Maxwell slot m
+template <int MODEL> __host__ __device__ constexpr int hm_mrow(int m) {   // conserved row of Maxwell slot m (B, E, psi, phi)
+  return m < 6 ? FSet<MODEL>::IB + m : (m == 6 ? FSet<MODEL>::IPSI : FSet<MODEL>::IPHI);
+}
 
 #ifndef RMHD_HM_GH
 #define RMHD_HM_GH 6     // reconstructions in flight per batch, role H (12 per face)
@@ -88,13 +90,17 @@ __host__ __device__ constexpr int hm_mrow(int m) { return m < 6 ? 5 + m : (m == 
 // the plane, and the marching axis ("z" below) is the grid's y axis: ZDIR = 1 selects the y components of the flux
 // vectors; the host passes ny = 1, nz = the grid's ny, bcz = its y boundary condition, hidz = 1/(2 dy).  A 2-D grid
 // then runs the same plane pipeline as a 3-D one instead of one isolated plane per CTA.
-template <bool HAS_Z, bool COMB = false, int TYP = 4, bool HAS_Y = true, int ZDIR = 2>
-__global__ void __launch_bounds__(HMGeom<TYP>::THREADS, TYP == 4 ? 2 : 1)
-k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int nx, int ny, int nz, int bcx, int bcy, int bcz,
+// MODEL = 1 (two-fluid, 10 hydro rows = 20 fields per face and axis): 32 x 4 tiles; the hydro role also carries 30 doubles of
+// z state, so a 3-D launch is held to one CTA per SM (168 registers), a 2-D one keeps two.
+template <bool HAS_Z, bool COMB = false, int TYP = 4, bool HAS_Y = true, int ZDIR = 2, int MODEL = 0>
+__global__ void __launch_bounds__(HMGeom<TYP, MODEL>::THREADS, MODEL == 0 ? (TYP == 4 ? 2 : 1) : (HAS_Z ? 1 : 2))
+k_flux_hm(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, size_t N, int nx, int ny, int nz, int bcx, int bcy, int bcz,
           double hidx, double hidy, double hidz, int seg_len, DevPar P, FluxComb cb) {
-  using FS = FSet<0>;
-  using SM = HMGeom<TYP>;
-  constexpr int NC = R_NC, NH = R_NH, NF = FS::NF, NHV = FS::NHV, NM = 8;
+  using FS = FSet<MODEL>;
+  using SM = HMGeom<TYP, MODEL>;
+  constexpr int NC = Dim<MODEL>::NC, NH = Dim<MODEL>::NH, NF = FS::NF, NHV = FS::NHV, NM = 8;
+  constexpr int NR = NHV > NM ? NHV : NM;           // rows a thread of either role can own
+  constexpr int GH = MODEL == 0 ? RMHD_HM_GH : 5;   // hydro reconstructions in flight per batch
   constexpr int TX = FF_TX, TY = TYP, XW = FF_XW, YR = SM::YR, MAIN = SM::MAIN, NT = SM::THREADS;
   constexpr int FSX = TY * XW, FSY = YR * TX;       // field strides of gX, gY
   extern __shared__ double sm[];
@@ -145,11 +151,11 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
   const int k0 = HAS_Z ? blockIdx.z * seg_len : 0;
   const int k1 = HAS_Z ? min(nz, k0 + seg_len) : 1;
   // z carry: pending left-biased reconstructions of the newest face, G of the previous face (own rows only)
-  double pend[NHV], Gprev[NM];                      // H uses pend[0..5], Gprev[0..5]; M uses pend[0..3], Gprev[0..7]
+  double pend[NHV], Gprev[NR];                      // H uses pend[0..5], Gprev[0..5]; M uses pend[0..3], Gprev[0..7]
 #pragma unroll
   for (int v = 0; v < NHV; ++v) pend[v] = 0.0;
 #pragma unroll
-  for (int v = 0; v < NM; ++v) Gprev[v] = 0.0;
+  for (int v = 0; v < NR; ++v) Gprev[v] = 0.0;
   int s_old = 0, s_new = 2 * NHV * MAIN;
 
   const int cbeg = HAS_Z ? k0 - 2 : 2, cend = HAS_Z ? k1 + 1 : 2;
@@ -158,9 +164,9 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
     const int k = HAS_Z ? c - 2 : 0;
     const bool do_xy = !HAS_Z || c >= k0 + 2;
     const unsigned pk = (unsigned)k * pstride;
-    double Lacc[NM];                                 // H: 6 rows (D, S, tau, rho_charge); M: 8 rows (B, E, psi, phi)
+    double Lacc[NR];                                 // H: 6 rows (D, S, tau, rho_charge); M: 8 rows (B, E, psi, phi)
 #pragma unroll
-    for (int v = 0; v < NM; ++v) Lacc[v] = 0.0;
+    for (int v = 0; v < NR; ++v) Lacc[v] = 0.0;
 
     if (roleH) {
       // ======================================= role H =======================================
@@ -169,7 +175,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
         if (inside) prefetch_rows<COMB, NHV>(cb, N, pk + (unsigned)j * nx + i, [](int h) { return FS::hv(h); });
         {
           double q_[NC], w_[NH], fh[NHV];
-          Com<0> cm;
+          Com<MODEL> cm;
           load_cell(pk + col_main, q_, w_);
           cell_common(q_, w_, P, cm);
           cell_hflux<0>(q_, w_, cm, P, fh);
@@ -192,7 +198,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
 #pragma unroll 1
         for (int t = 0; t < (HAS_Y ? 2 : 1); ++t) {
           double o[2 * NHV];
-          face_recon_range<0, 2 * NHV, RMHD_HM_GH>(t ? gY + ty * TX + lane : gX + ty * XW + lane, t ? FSY : FSX, t ? TX : 1, o);
+          face_recon_range<MODEL, 0, 2 * NHV, GH>(t ? gY + ty * TX + lane : gX + ty * XW + lane, t ? FSY : FSX, t ? TX : 1, o);
           if (t == 0) {
 #pragma unroll
             for (int h = 0; h < NHV; ++h) {
@@ -215,7 +221,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
         double u0[2 * NHV];
         {
           double q_[NC], w_[NH], fh[NHV];
-          Com<0> cm;
+          Com<MODEL> cm;
           load_cell((unsigned)bc_map(c, nz, bcz) * pstride + col_main, q_, w_);
           cell_common(q_, w_, P, cm);
           cell_hflux<ZDIR>(q_, w_, cm, P, fh);
@@ -225,8 +231,8 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
         if (c >= k0) {
           double o[2 * NHV];
 #pragma unroll
-          for (int f0 = 0; f0 < 2 * NHV; f0 += RMHD_HM_GH) {
-            constexpr int G = RMHD_HM_GH;
+          for (int f0 = 0; f0 < 2 * NHV; f0 += GH) {
+            constexpr int G = GH;
             double a[G], b[G], cc[G];
 #pragma unroll
             for (int g = 0; g < G; ++g) {
@@ -267,7 +273,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
       // z first: it loads B, E, psi, phi of planes c-2, c-1, c; plane c-2 IS plane k, so the x/y fields of the own
       // cell are built from the same registers (no second load)
       if (do_xy) {
-        if (inside) prefetch_rows<COMB, NM>(cb, N, pk + (unsigned)j * nx + i, [](int m) { return hm_mrow(m); });
+        if (inside) prefetch_rows<COMB, NM>(cb, N, pk + (unsigned)j * nx + i, [](int m) { return hm_mrow<MODEL>(m); });
         if (HAS_Z && c < cend) {
           const unsigned pn = (unsigned)(k + 1) * pstride;
           if (HAS_Y && (TY == 4 || ty < 4)) prefetch_cell(pn + col_yh);
@@ -313,18 +319,18 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
       if (do_xy) {
         {
           double q_[NC], w_[NH], g[NF];
-          Com<0> cm;
+          Com<MODEL> cm;
           if (HAS_Y && (TY == 4 || ty < 4)) {        // the 4 y-halo rows: M warps 0-3
             load_cell(pk + col_yh, q_, w_);
             cell_common(q_, w_, P, cm);
-            cell_fields<0, 1>(q_, w_, cm, P, g);
+            cell_fields<MODEL, 1>(q_, w_, cm, P, g);
 #pragma unroll
             for (int f = 0; f < NF; ++f) gY[(f * YR + hrow) * TX + lane] = g[f];
           }
           if (wrp == 2 * TY - 1 && lane < 4 * TY) {
             load_cell(pk + col_xh, q_, w_);
             cell_common(q_, w_, P, cm);
-            cell_fields<0, 0>(q_, w_, cm, P, g);
+            cell_fields<MODEL, 0>(q_, w_, cm, P, g);
 #pragma unroll
             for (int f = 0; f < NF; ++f) gX[(f * TY + xh_row) * XW + xh_col] = g[f];
           }
@@ -340,7 +346,7 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
           const bool ydir = t == 1 || (t == 2 && wrp == TY + XB);
           const double* p = t == 0 ? gX + ty * XW + lane : (t == 1 ? gY + ty * TX + lane : (ydir ? gY + TY * TX + lane : gX + lane * XW + TX));
           double o[NM], G[NM];
-          face_recon_range<2 * NHV, NM, NM>(p, ydir ? FSY : FSX, ydir ? TX : 1, o);
+          face_recon_range<MODEL, 2 * NHV, NM, NM>(p, ydir ? FSY : FSX, ydir ? TX : 1, o);
           if (ydir) assemble_M<1>(o, G); else assemble_M<0>(o, G);
           if (t == 0) {
 #pragma unroll
@@ -350,19 +356,19 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
             }
           } else if (t == 1) {
 #pragma unroll
-            for (int v = 0; v < NM; ++v) { fY[(hm_mrow(v) * (TY + 1) + ty) * TX + lane] = G[v]; Lacc[v] = fma(G[v], hidy, Lacc[v]); }
+            for (int v = 0; v < NM; ++v) { fY[(hm_mrow<MODEL>(v) * (TY + 1) + ty) * TX + lane] = G[v]; Lacc[v] = fma(G[v], hidy, Lacc[v]); }
           } else if (ydir) {
 #pragma unroll
-            for (int v = 0; v < NM; ++v) fY[(hm_mrow(v) * (TY + 1) + TY) * TX + lane] = G[v];
+            for (int v = 0; v < NM; ++v) fY[(hm_mrow<MODEL>(v) * (TY + 1) + TY) * TX + lane] = G[v];
           } else if (lane < TY) {
 #pragma unroll
-            for (int v = 0; v < NM; ++v) fX[hm_mrow(v) * TY + lane] = G[v];
+            for (int v = 0; v < NM; ++v) fX[hm_mrow<MODEL>(v) * TY + lane] = G[v];
           }
         }
         if ((HAS_Y && wrp == TY + XB + 2) || wrp == TY + XB + 3) {   // the same two extra face sets of the hydro rows (12 fields), taken off role H
           const bool ydir = wrp == TY + XB + 2;
           double o[2 * NHV];
-          face_recon_range<0, 2 * NHV, RMHD_HM_GH>(ydir ? gY + TY * TX + lane : gX + (lane & (TY - 1)) * XW + TX, ydir ? FSY : FSX, ydir ? TX : 1, o);
+          face_recon_range<MODEL, 0, 2 * NHV, GH>(ydir ? gY + TY * TX + lane : gX + (lane & (TY - 1)) * XW + TX, ydir ? FSY : FSX, ydir ? TX : 1, o);
           if (ydir) {
 #pragma unroll
             for (int h = 0; h < NHV; ++h) fY[(FS::hv(h) * (TY + 1) + TY) * TX + lane] = o[h] + o[NHV + h];
@@ -374,14 +380,14 @@ k_flux_hm(ConsRows<0> qin, HydRows<0> win, double* __restrict__ L, size_t N, int
         mbar_arrive(&bar2);
         mbar_wait(&bar2, ph2); ph2 ^= 1u;
 #pragma unroll
-        for (int v = 0; v < NM; ++v) if (HAS_Y) Lacc[v] = fma(-fY[(hm_mrow(v) * (TY + 1) + ty + 1) * TX + lane], hidy, Lacc[v]);
+        for (int v = 0; v < NM; ++v) if (HAS_Y) Lacc[v] = fma(-fY[(hm_mrow<MODEL>(v) * (TY + 1) + ty + 1) * TX + lane], hidy, Lacc[v]);
         if (lane == 31) {
 #pragma unroll
-          for (int v = 0; v < NM; ++v) Lacc[v] = fma(-fX[hm_mrow(v) * TY + ty], hidx, Lacc[v]);
+          for (int v = 0; v < NM; ++v) Lacc[v] = fma(-fX[hm_mrow<MODEL>(v) * TY + ty], hidx, Lacc[v]);
         }
         if (inside) {
           const unsigned id = pk + (unsigned)j * nx + i;
-          store_rows<COMB, NM>(L, cb, N, id, Lacc, [](int m) { return hm_mrow(m); });
+          store_rows<COMB, NM>(L, cb, N, id, Lacc, [](int m) { return hm_mrow<MODEL>(m); });
         }
       }
     }

@@ -158,13 +158,12 @@ template <int MODEL, bool HAS_Z, bool COMB, int TYP>
 int launch_flux_fused(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODEL>& wr, double* L, const FluxComb& cb) {
   static bool attr_set[8] = {false, false, false, false, false, false, false, false};
   const int nx = c->n[0], ny = c->n[1], nz = c->n[2];
-  bool two_role = false;
-  if constexpr (MODEL == 0) two_role = !c->one_role;
+  const bool two_role = !c->one_role;
   const int ty = two_role ? TYP : FF_TY;
-  const size_t smem = two_role ? HMGeom<TYP>::bytes(HAS_Z) : FFSmem<MODEL>::bytes(HAS_Z);
+  const size_t smem = two_role ? HMGeom<TYP, MODEL>::bytes(HAS_Z) : FFSmem<MODEL>::bytes(HAS_Z);
   if (!attr_set[c->device & 7]) {
     CK(c, cudaFuncSetAttribute(k_flux_fused<MODEL, HAS_Z, COMB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFSmem<MODEL>::bytes(HAS_Z)));
-    if constexpr (MODEL == 0) CK(c, cudaFuncSetAttribute(k_flux_hm<HAS_Z, COMB, TYP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)HMGeom<TYP>::bytes(HAS_Z)));
+    CK(c, cudaFuncSetAttribute(k_flux_hm<HAS_Z, COMB, TYP, true, 2, MODEL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)HMGeom<TYP, MODEL>::bytes(HAS_Z)));
     attr_set[c->device & 7] = true;
   }
   const int gx = (nx + FF_TX - 1) / FF_TX, gy = (ny + ty - 1) / ty;
@@ -172,7 +171,8 @@ int launch_flux_fused(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODE
   if (HAS_Z) {
     // z segments: pick the count (segments of >= 16 planes) that wastes least, counting the partially filled
     // last wave of resident CTAs and the 4 feed-only prologue planes of every segment
-    const long long tiles = (long long)gx * gy, slots = (two_role && TYP == 8 ? 1LL : 2LL) * c->sm_count;
+    const bool one_cta = two_role && (TYP == 8 || MODEL == 1);
+    const long long tiles = (long long)gx * gy, slots = (one_cta ? 1LL : 2LL) * c->sm_count;
     double best = 1e300;
     for (int s = 1; s <= (nz + 15) / 16 && s <= 64; ++s) {
       const int len = (nz + s - 1) / s, cnt = (nz + len - 1) / len;
@@ -183,12 +183,10 @@ int launch_flux_fused(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODE
   }
   dim3 grid(gx, gy, nseg);
   Timed t(c, KC_FLUX);
-  if constexpr (MODEL == 0) {
-    if (two_role)
-      k_flux_hm<HAS_Z, COMB, TYP><<<grid, HMGeom<TYP>::THREADS, smem, c->stream>>>(qr, wr, L, c->N, nx, ny, nz, c->p.bc[0], c->p.bc[1], c->p.bc[2],
-                                                                                 0.5 / c->dx[0], 0.5 / c->dx[1], 0.5 / c->dx[2], seg_len, c->P, cb);
-  }
-  if (!two_role)
+  if (two_role)
+    k_flux_hm<HAS_Z, COMB, TYP, true, 2, MODEL><<<grid, HMGeom<TYP, MODEL>::THREADS, smem, c->stream>>>(
+        qr, wr, L, c->N, nx, ny, nz, c->p.bc[0], c->p.bc[1], c->p.bc[2], 0.5 / c->dx[0], 0.5 / c->dx[1], 0.5 / c->dx[2], seg_len, c->P, cb);
+  else
     k_flux_fused<MODEL, HAS_Z, COMB><<<grid, FF_THREADS, smem, c->stream>>>(qr, wr, L, c->N, nx, ny, nz, c->p.bc[0], c->p.bc[1], c->p.bc[2],
                                                                            0.5 / c->dx[0], 0.5 / c->dx[1], 0.5 / c->dx[2], seg_len, c->P, cb);
   CK(c, cudaGetLastError());
@@ -196,7 +194,9 @@ int launch_flux_fused(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODE
 }
 template <int MODEL, bool HAS_Z, bool COMB>
 int launch_flux_fused(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODEL>& wr, double* L, const FluxComb& cb) {
-  if (MODEL == 0 && c->hm_ty == 8) return launch_flux_fused<MODEL, HAS_Z, COMB, 8>(c, qr, wr, L, cb);
+  if constexpr (MODEL == 0) {
+    if (c->hm_ty == 8) return launch_flux_fused<MODEL, HAS_Z, COMB, 8>(c, qr, wr, L, cb);
+  }
   return launch_flux_fused<MODEL, HAS_Z, COMB, 4>(c, qr, wr, L, cb);
 }
 
@@ -209,7 +209,7 @@ int launch_flux_march2d(rmhd_ctx* c, const ConsRows<0>& qr, const HydRows<0>& wr
   const int nx = c->n[0], ny = c->n[1];
   const size_t smem = HMGeom<TYP>::bytes(true);
   if (!attr_set[c->device & 7]) {
-    CK(c, cudaFuncSetAttribute(k_flux_hm<true, COMB, TYP, false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CK(c, cudaFuncSetAttribute(k_flux_hm<true, COMB, TYP, false, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     attr_set[c->device & 7] = true;
   }
   const int gx = (nx + FF_TX * TYP - 1) / (FF_TX * TYP);
@@ -227,7 +227,7 @@ int launch_flux_march2d(rmhd_ctx* c, const ConsRows<0>& qr, const HydRows<0>& wr
   }
   dim3 grid(gx, 1, nseg);
   Timed t(c, KC_FLUX);
-  k_flux_hm<true, COMB, TYP, false, 1><<<grid, HMGeom<TYP>::THREADS, smem, c->stream>>>(
+  k_flux_hm<true, COMB, TYP, false, 1, 0><<<grid, HMGeom<TYP>::THREADS, smem, c->stream>>>(
       qr, wr, L, c->N, nx, 1, ny, c->p.bc[0], 0, c->p.bc[1], 0.5 / c->dx[0], 0.0, 0.5 / c->dx[1], seg_len, c->P, cb);
   CK(c, cudaGetLastError());
   return RMHD_OK;
