@@ -118,6 +118,8 @@ def make_workload(name, synth):
         return synth.khi_paper(model=0)
     if name == "khi2f":             # ... two-fluid
         return synth.khi_paper(model=1)
+    if name == "tf3d":              # 3-D two-fluid blast, 128^3 (kernel studies; not a BASELINE config)
+        return synth.two_fluid_blast(n=128)
     raise SystemExit(f"unknown workload {name}")
 
 

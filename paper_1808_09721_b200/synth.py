@@ -196,6 +196,24 @@ def khi_paper(model=RESISTIVE, nx=512, ny=1024, nsteps=None, cfl=0.4, integrator
                 rho_charge=None, nsteps=nsteps, tol=1e-8)
 
 
+def two_fluid_blast(n=128, nsteps=10, integrator="ssp2"):
+    """3-D two-fluid pair-plasma blast: the recipe of BASELINE.json configs[4] (3-D resistive blast) carried over to the
+    18-variable model (not a BASELINE config; exercises the 3-D two-fluid kernels).  rho_e = rho_p = 0.5, total
+    p = 1 inside r < 0.1 (cell-centre radius) and 0.01 outside split equally, both species at rest, B = (0.1, 0, 0), E = 0,
+    mu_p = -mu_e = 100, eta = 1e-3, Gamma = 4/3, CFL 0.3, outflow."""
+    c = cell_centres(n, -0.5, 0.5)
+    r2 = c[:, None, None] ** 2 + c[None, :, None] ** 2 + c[None, None, :] ** 2
+    w = np.zeros((16, n, n, n))
+    for sp in range(2):
+        w[5 * sp] = 0.5
+        w[5 * sp + 4] = 0.5 * np.where(r2 < 0.1 ** 2, 1.0, 0.01)
+    w[10] = 0.1
+    params = dict(model=TWO_FLUID, nx=n, ny=n, nz=n, ng=4, xlim=(-0.5, 0.5), ylim=(-0.5, 0.5), zlim=(-0.5, 0.5),
+                  bc=(BC_OUTFLOW,) * 3, gamma=4.0 / 3.0, eta=1e-3, mu_e=-100.0, mu_p=100.0, kappa=1.0, cfl=0.3,
+                  integrator=integrator)
+    return dict(name="two_fluid_blast", params=params, prims=w, rho_charge=None, nsteps=nsteps, tol=1e-8)
+
+
 def random_resistive_prims(n, seed, vmax=0.99, with_E=True):
     """Random admissible resistive primitive states (round-trip pins, kernel unit tests)."""
     rng = np.random.default_rng(seed)

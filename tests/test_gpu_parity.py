@@ -415,3 +415,16 @@ def test_paper_setups_parity(B, O, synth, case, integrator):
     assert rel_l1(q, qo) <= tol, rel_l1(q, qo)
     nh = 5 if c["params"]["model"] == 0 else 10
     assert rel_l1(w[:nh], wo[:nh]) <= 10 * tol
+
+
+@pytest.mark.parametrize("integrator,flux", [("ssp2", None), ("ssp3", None), ("ssp2", "fused1"), ("ssp2", "split")])
+def test_two_fluid_3d_blast_parity(B, O, synth, integrator, flux, monkeypatch):
+    """Full steps of the 18-variable model in 3-D (two-role flux kernel, one-role kernel, per-axis kernels)."""
+    if flux:
+        monkeypatch.setenv("RMHD_FLUX", flux)
+    c = synth.two_fluid_blast(n=36, nsteps=8, integrator=integrator)
+    q, w, st = run_gpu(B, c)
+    qo, wo, sto = run_oracle(O, c)
+    assert st["n_failed"] == 0 and sto["n_failed"] == 0
+    assert rel_l1(q, qo) <= 1e-8, rel_l1(q, qo)
+    assert rel_l1(w[:10], wo[:10]) <= 1e-8
