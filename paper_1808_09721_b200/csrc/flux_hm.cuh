@@ -93,7 +93,7 @@ template <int MODEL> __host__ __device__ constexpr int hm_mrow(int m) {   // con
 // MODEL = 1 (two-fluid, 10 hydro rows = 20 fields per face and axis): 32 x 4 tiles; the hydro role also carries 30 doubles of
 // z state, so a 3-D launch is held to one CTA per SM (168 registers), a 2-D one keeps two.
 template <bool HAS_Z, bool COMB = false, int TYP = 4, bool HAS_Y = true, int ZDIR = 2, int MODEL = 0>
-__global__ void __launch_bounds__(HMGeom<TYP, MODEL>::THREADS, MODEL == 0 ? (TYP == 4 ? 2 : 1) : (HAS_Z ? 1 : 2))
+__global__ void __launch_bounds__(HMGeom<TYP, MODEL>::THREADS, MODEL == 0 ? (TYP == 4 ? 2 : 1) : ((HAS_Z || TYP == 8) ? 1 : 2))
 k_flux_hm(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, size_t N, int nx, int ny, int nz, int bcx, int bcy, int bcz,
           double hidx, double hidy, double hidz, int seg_len, DevPar P, FluxComb cb) {
   using FS = FSet<MODEL>;

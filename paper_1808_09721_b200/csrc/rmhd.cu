@@ -194,7 +194,7 @@ int launch_flux_fused(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODE
 }
 template <int MODEL, bool HAS_Z, bool COMB>
 int launch_flux_fused(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODEL>& wr, double* L, const FluxComb& cb) {
-  if constexpr (MODEL == 0) {
+  if constexpr (MODEL == 0 || !HAS_Z) {     // 32 x 8 tiles: resistive always, two-fluid in 2-D (its 3-D ring does not fit)
     if (c->hm_ty == 8) return launch_flux_fused<MODEL, HAS_Z, COMB, 8>(c, qr, wr, L, cb);
   }
   return launch_flux_fused<MODEL, HAS_Z, COMB, 4>(c, qr, wr, L, cb);
