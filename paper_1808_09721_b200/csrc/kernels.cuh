@@ -60,7 +60,7 @@ __global__ void __launch_bounds__(256) k_set_initial(const double* __restrict__ 
                                                      double* __restrict__ q, double* __restrict__ w, size_t N, int nx, int ny, int nz,
                                                      int bcx, int bcy, int bcz, double i2dx, double i2dy, double i2dz,
                                                      DevPar P, Stats* st) {
-  constexpr int NC = Dim<MODEL>::NC, NH = Dim<MODEL>::NH, NP = Dim<MODEL>::NP;
+  constexpr int NC = Dim<MODEL>::NC, NH = Dim<MODEL>::NH;
   const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= N) return;
   double wl[NH], B[3], E[3], ql[NC];
