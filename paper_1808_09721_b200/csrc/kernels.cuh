@@ -444,11 +444,13 @@ __global__ void __launch_bounds__(FLUX_THREADS, 2) k_flux(ConsRows<MODEL> qin, H
   const int ns = AXIS == 0 ? nx : (AXIS == 1 ? ny : nz);
   const int no = AXIS == 0 ? ny * nz : nx;
   const int o0 = blockIdx.x * TO;
-  const int s0 = blockIdx.y * TS;
+  // a 1-D grid (AXIS 0, one row) lays the TO tile rows along x: row o covers cells s0 + o TS ... (all threads busy)
+  const bool rows_x = AXIS == 0 && no == 1;
+  const int s0 = rows_x ? blockIdx.y * (TS * TO) : blockIdx.y * TS;
   const int third = blockIdx.z;
 
   // ---- L2 prefetch of the tile that the CTA about one wave behind this one will stage (AXIS 0 only)
-  if (AXIS == 0) {
+  if (AXIS == 0 && !rows_x) {
     const long long lin = (long long)blockIdx.x + (long long)gridDim.x * blockIdx.y + FLUX_PREFETCH_CTAS;
     if (lin < (long long)gridDim.x * gridDim.y && tid < CS) {
       const int pbx = (int)(lin % gridDim.x), pby = (int)(lin / gridDim.x);
@@ -466,8 +468,8 @@ __global__ void __launch_bounds__(FLUX_THREADS, 2) k_flux(ConsRows<MODEL> qin, H
   for (int item = tid; item < CS; item += FLUX_THREADS) {
     int sh, o;
     if (AXIS == 0) { sh = item % (TS + 4); o = item / (TS + 4); } else { o = item % TO; sh = item / TO; }
-    const int c = s0 - 2 + sh;
-    const int oo = o0 + o;
+    const int c = s0 - 2 + sh + (rows_x ? o * TS : 0);
+    const int oo = rows_x ? 0 : o0 + o;
     if (c < ns + 2 && oo < no) {
       const int cm = bc_map(c, ns, bc);
       size_t idx;
@@ -511,8 +513,8 @@ __global__ void __launch_bounds__(FLUX_THREADS, 2) k_flux(ConsRows<MODEL> qin, H
     int s, o, fi, st;
     if (AXIS == 0) { s = tid % TS; o = tid / TS; fi = o * (TS + 1) + s; st = 1; }
     else { o = tid % TO; s = tid / TO; fi = s * TO + o; st = TO; }
-    const int c = s0 + s;
-    const int oo = o0 + o;
+    const int c = s0 + s + (rows_x ? o * TS : 0);
+    const int oo = rows_x ? 0 : o0 + o;
     if (c < ns && oo < no) {
       size_t idx;
       if (AXIS == 0) idx = (size_t)oo * nx + c;

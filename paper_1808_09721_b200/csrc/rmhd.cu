@@ -127,6 +127,7 @@ int launch_flux_axis(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODEL
       attr_set[c->device & 7] = true;
     }
     dim3 grid((ny * nz + TO - 1) / TO, (ns + TS - 1) / TS, 1);
+    if (ny * nz == 1) grid = dim3(1, (ns + TS * TO - 1) / (TS * TO), 1);   // 1-D: the tile rows are laid along x
     Timed t(c, KC_FLUX);
     k_flux<MODEL, AXIS><<<grid, FLUX_THREADS, smem, c->stream>>>(qr, wr, L, c->N, nx, ny, nz, c->p.bc[AXIS], 1.0 / c->dx[AXIS], accumulate, c->P);
     CK(c, cudaGetLastError());
