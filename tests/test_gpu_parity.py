@@ -428,3 +428,47 @@ def test_two_fluid_3d_blast_parity(B, O, synth, integrator, flux, monkeypatch):
     assert st["n_failed"] == 0 and sto["n_failed"] == 0
     assert rel_l1(q, qo) <= 1e-8, rel_l1(q, qo)
     assert rel_l1(w[:10], wo[:10]) <= 1e-8
+
+
+def test_nonconvergence_is_reported_not_hidden(B, synth):
+    """max_iter_stage = 1 on a stiff tube (sigma dt = 9): the Newton loops cannot finish.  rmhd_step still advances the
+    requested steps, returns RMHD_ERR_NONCONVERGED, and get_stats names the count and the first failing cell
+    (include/rmhd.h error contract; SURVEY.md section 5 'failure detection')."""
+    c = synth.config1()
+    kw = dict(c["params"]); kw["max_iter_stage"] = 1
+    sim = B.Rmhd(**kw); sim.set_initial(np.ascontiguousarray(c["prims"]))
+    rc = sim.step(3, check=False)
+    assert rc == B.RMHD_ERR_NONCONVERGED
+    assert abs(sim.time - 3 * sim.dt) < 1e-15
+    st = sim.stats()
+    assert st["n_failed"] > 0 and 0 <= st["first_failed_cell"] < 128
+    # every solve stopped after its single iteration (or, in a cell an earlier failure made inadmissible, before it)
+    assert st["hist_stage"][:2].sum() == st["hist_stage"].sum() == 2 * 3 * 128 and st["hist_stage"][1] > 700
+    with pytest.raises(B.RmhdError) as e:
+        sim.step(1)
+    assert e.value.code == B.RMHD_ERR_NONCONVERGED
+    sim.close()
+    # the same run with the default cap converges everywhere
+    sim = B.Rmhd(**c["params"]); sim.set_initial(np.ascontiguousarray(c["prims"])); sim.step(3)
+    assert sim.stats()["n_failed"] == 0
+    sim.close()
+
+
+def test_stage_batch_flags_inadmissible_cells_like_the_oracle(B, O, synth):
+    """config 2 recipe with E perturbations 10x larger (std 0.1): some low-pressure, strong-field cells have no
+    admissible root.  Both sides must flag (almost) the same cells and agree on all the others."""
+    n = 2 ** 15
+    c = synth.config2(n, seed=0)
+    w = c["prims"].copy()
+    rng = np.random.default_rng(123)
+    w[8:11] += 0.1 * rng.standard_normal((3, n))
+    P = B.make_params(**c["params"]); PO = O.make_params(**c["params"])
+    q_ex = O.prim2cons(PO, w)
+    qo, wo, ito, flo = O.stage_batch(PO, q_ex, w, c["a_dt"], c["sigma_cell"])
+    q = np.empty_like(q_ex); wg = np.empty_like(w); it = np.zeros(n, np.int32); fl = np.zeros(n, np.int32)
+    B.rmhd_stage_batch(P, q_ex, w, c["a_dt"], q, wg, c["sigma_cell"], it, fl)
+    bad, bado = fl != 0, flo != 0
+    assert (bad != bado).sum() <= max(2, 0.02 * max(bad.sum(), bado.sum()))      # the same cells, up to marginal ones
+    ok = ~bad & ~bado
+    assert ok.mean() > 0.9
+    assert rel_l1(q[:, ok], qo[:, ok]) <= 1e-10
