@@ -312,7 +312,12 @@ def run_ours(args):
     roof["kernel_time_shares"] = shares
     # the minimum for the SSP2(222) step, whatever the kernel split; SSP3(332) by the same rules:
     # S1 29 + F1 33 + S2 57 + F2 33 + S3 76 + (F3 + C + P fused) 95
-    step_alg_bytes = (323 if nstage == 3 else 195) * 8 * ncell
+    # two-fluid (18 cons, 10 prims, 9 source rows) by the same rules: 47 + 46 + 83 + 110 = 286; SSP3: + 46 + 110 + (137 - 110) = 469
+    if p["model"] == 0:
+        step_doubles = 323 if nstage == 3 else 195
+    else:
+        step_doubles = 469 if nstage == 3 else 286
+    step_alg_bytes = step_doubles * 8 * ncell
     roof["whole_step_hbm_frac"] = step_alg_bytes / (ms_total / args.steps * 1e-3) * 1e-9 / hbm_peak
 
     # ---- end to end through the C-ABI with host buffers ---------------------------------------
