@@ -2,7 +2,7 @@
 // rmhd_oracle.cpp -- CPU ORACLE.  TEST INFRASTRUCTURE ONLY.
 //
 // A plain, slow, serial-by-construction (optionally OpenMP over independent cells) FP64
-// implementation of one step of the finite-volume IMEX SSP2(222) scheme for resistive
+// implementation of one step of the finite-volume IMEX SSP2(222) / SSP3(332) schemes for resistive
 // single-fluid (14 conserved variables) and two-fluid (18) special-relativistic MHD of
 // Wright & Hawke, "Resistive and multi-fluid RMHD on graphics processing units".
 //
@@ -18,7 +18,10 @@
 // wave (Maxwell flux signs); uniform state => L == 0; telescoping conservation; closed
 // form stage solution and SSP2(222) stability function R(z); stage residual; frozen-v
 // guess vs Sherman-Morrison; steady states; bitwise mirror symmetry; self-similar current
-// sheet; ideal limit; two-fluid Langmuir frequency.  Full configs 1,3,4,5
+// sheet; ideal limit; two-fluid Langmuir frequency; general IMEX stepper and
+// SSP3(332) (Table 3): order conditions, implicit stability function, Shu-Osher
+// RK3 recomposition through eval_L, telegraph-mode closed form, Table 2 through the general
+// stepper against the SSP2(222) path, second-order convergence.  Full configs 1,3,4,5
 // have no printed reference values in the paper: "parity unpinned" beyond those pins.
 //
 // Build: g++ -O2 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/build.py).
