@@ -278,8 +278,8 @@ def run_ours(args):
     nfl = max(kt["flux"]["launches"], 1) / (float(nstage) * args.steps)   # launches per L(q): 1 fused, naxes split
     alg_bytes = {
         "stage1": 34 * 8 * ncell,                                   # R qn 14 + w 5; W E*,psi*,phi* 5 + w 5 + Psi1 5
-        "stage2": (71 if fused else 62) * 8 * ncell,                # R qn 14 + L1 14 + Psi1 5 + w 5; W q2 14 + w 5 + (A 14 | Psi2 5)
-        "flux": ((33 * (nstage - 1) + 47) / float(nstage) if fused else 33 / nfl) * 8 * ncell,   # F: R 19, W 14; fused last F: R 19 + A 14, W 14
+        "stage2": 62 * 8 * ncell,                                   # R qn 14 + L1 14 + Psi1 5 + w 5; W q2 14 + w 5 + (A, source rows 5 | Psi2 5)
+        "flux": ((33 * (nstage - 1) + 47) / float(nstage) if fused else 33 / nfl) * 8 * ncell,   # F: R 19, W 14; fused last F: R 19 + qn 9 + A 5, W 14
         "combine_c2p": (21 if fused else 76) * 8 * ncell,           # fused: con2prim R 11 + 5, W 5; else k_final R 57, W 19
     }
     peak_tf = SM_COUNT * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 * 1e-12
@@ -302,7 +302,7 @@ def run_ours(args):
         roof = {"bound": "hbm", "kernel": dom, "achieved": alg_bytes[dom] / (avg_ms * 1e-3) * 1e-9, "peak": hbm_peak,
                 "unit": "GB/s", "peak_source": peak_src + " (MEASURED_PEAKS.json hbm_gbs)", "traffic": None}
     # DRAM bytes per launch of that kernel from the committed `ncu --set full` capture (profiles/r1e_kernels.md:
-    # dram__bytes_read.sum + dram__bytes_write.sum; F1 4.589 GB, F2 6.509 GB, S1 4.517, S2 9.498, P 2.790), cfg5 / SSP2(222) only
+    # dram__bytes_read.sum + dram__bytes_write.sum; F1 4.589 GB, F2 6.509 GB, S1 4.517, S2 9.498 before A shrank to its 5 source rows, P 2.790), cfg5 / SSP2(222) only
     ncu_traffic = {"flux": 0.5 * (4.589e9 + 6.509e9), "stage1": 4.517e9, "stage2": 9.498e9, "combine_c2p": 2.790e9}
     if args.workload == "cfg5" and nstage == 2 and fused:
         roof["traffic"] = ncu_traffic[dom]

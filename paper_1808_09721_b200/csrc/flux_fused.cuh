@@ -187,26 +187,44 @@ template <int MODEL> struct FFSmem {
 //   q^{n+1}_v = A_v + hdt L2_v,   A_v = qn_v + hdt L1_v + hdt (Psi1_v + Psi2_v) left by stage 2 in the L2 buffer,
 //   hdt = dt/2 (w = w~ = (1/2, 1/2), Table 2),
 // into the qn rows (F2 reads the stage state qs, never qn), so L2 is neither written nor re-read.
-struct FluxComb { double* q; const double* A; double hdt; };
+// theta > 0: for the rows WITHOUT a source the last stage is q_last = qn + c (sum of the earlier L), so their part of eq (11)
+// is A_v = (1 - theta) qn_v + theta q_last,v (SSP2(222): theta = 1/2; SSP3(332): theta = 2/3) and the stage kernel stores A
+// only for the rows with a source; q_last is this launch's own input (qs).
+struct FluxComb { double* q; const double* A; double hdt; const double* qs; double theta; };
+template <int MODEL> __host__ __device__ constexpr bool has_source(int v) {
+  return MODEL == 0 ? ((v >= 8 && v <= 10) || v >= 12) : ((v >= 6 && v <= 9) || v >= 13);
+}
 // store NR rows (row index by ROW(r)) of one cell: L itself, or the eq-(11) update
-template <bool COMB, int NR, class ROW>
+template <bool COMB, int NR, int MODEL, class ROW>
 RMHD_DEV void store_rows(double* __restrict__ L, const FluxComb& cb, size_t N, unsigned id, const double* Lacc, ROW row) {
   if constexpr (!COMB) {
 #pragma unroll
     for (int r = 0; r < NR; ++r) (L + (size_t)row(r) * N)[id] = Lacc[r];
   } else {
-    double x[NR];
+    double x[NR], y[NR];
+    const bool mix = cb.theta > 0.0;
 #pragma unroll
-    for (int r = 0; r < NR; ++r) x[r] = __ldg((cb.A + (size_t)row(r) * N) + id);
+    for (int r = 0; r < NR; ++r) {
+      const size_t o = (size_t)row(r) * N;
+      if (mix && !has_source<MODEL>(row(r))) { x[r] = (cb.q + o)[id]; y[r] = __ldg((cb.qs + o) + id); }
+      else { x[r] = __ldg((cb.A + o) + id); y[r] = 0.0; }
+    }
 #pragma unroll
-    for (int r = 0; r < NR; ++r) (cb.q + (size_t)row(r) * N)[id] = fma(cb.hdt, Lacc[r], x[r]);
+    for (int r = 0; r < NR; ++r) {
+      const double a = (mix && !has_source<MODEL>(row(r))) ? fma(cb.theta, y[r] - x[r], x[r]) : x[r];
+      (cb.q + (size_t)row(r) * N)[id] = fma(cb.hdt, Lacc[r], a);
+    }
   }
 }
-template <bool COMB, int NR, class ROW>
+template <bool COMB, int NR, int MODEL, class ROW>
 RMHD_DEV void prefetch_rows(const FluxComb& cb, size_t N, unsigned id, ROW row) {
   if constexpr (COMB) {
+    const bool mix = cb.theta > 0.0;
 #pragma unroll
-    for (int r = 0; r < NR; ++r) prefetch_l2((cb.A + (size_t)row(r) * N) + id);
+    for (int r = 0; r < NR; ++r) {
+      const size_t o = (size_t)row(r) * N;
+      prefetch_l2(((mix && !has_source<MODEL>(row(r))) ? (const double*)cb.q : cb.A) + o + id);
+    }
   }
 }
 
@@ -267,7 +285,7 @@ k_flux_fused(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, si
     if (do_xy) {
       const size_t pk = (size_t)k * pstride;
       // ---------------- P1: fields of the tile and its halo -> shared memory ------------------------
-      if (inside) prefetch_rows<COMB, NC>(cb, N, (unsigned)(pk + (size_t)j * nx + i), [](int r) { return r; });
+      if (inside) prefetch_rows<COMB, NC, MODEL>(cb, N, (unsigned)(pk + (size_t)j * nx + i), [](int r) { return r; });
       if (HAS_Z && c < cend) {                      // L2 prefetch of what the next iteration loads first
         const size_t pn = (size_t)(k + 1) * pstride;
         if (is_main) { prefetch_cell(pn + col_yh); prefetch_cell((size_t)bc_map(c + 1, nz, bcz) * pstride + col_main); }
@@ -395,7 +413,7 @@ k_flux_fused(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, si
     }
     if (do_xy && inside) {
       const size_t id = (size_t)k * pstride + (size_t)j * nx + i;
-      store_rows<COMB, NC>(L, cb, N, (unsigned)id, Lacc, [](int r) { return r; });
+      store_rows<COMB, NC, MODEL>(L, cb, N, (unsigned)id, Lacc, [](int r) { return r; });
     }
   }
 }

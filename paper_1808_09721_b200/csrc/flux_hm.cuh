@@ -172,7 +172,7 @@ k_flux_hm(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, size_
       // ======================================= role H =======================================
       if (do_xy) {
         if (HAS_Z && c < cend) prefetch_cell((unsigned)bc_map(c + 1, nz, bcz) * pstride + col_main);
-        if (inside) prefetch_rows<COMB, NHV>(cb, N, pk + (unsigned)j * nx + i, [](int h) { return FS::hv(h); });
+        if (inside) prefetch_rows<COMB, NHV, MODEL>(cb, N, pk + (unsigned)j * nx + i, [](int h) { return FS::hv(h); });
         {
           double q_[NC], w_[NH], fh[NHV];
           Com<MODEL> cm;
@@ -265,7 +265,7 @@ k_flux_hm(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, size_
         }
         if (inside) {
           const unsigned id = pk + (unsigned)j * nx + i;
-          store_rows<COMB, NHV>(L, cb, N, id, Lacc, [](int h) { return FS::hv(h); });
+          store_rows<COMB, NHV, MODEL>(L, cb, N, id, Lacc, [](int h) { return FS::hv(h); });
         }
       }
     } else {
@@ -273,7 +273,7 @@ k_flux_hm(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, size_
       // z first: it loads B, E, psi, phi of planes c-2, c-1, c; plane c-2 IS plane k, so the x/y fields of the own
       // cell are built from the same registers (no second load)
       if (do_xy) {
-        if (inside) prefetch_rows<COMB, NM>(cb, N, pk + (unsigned)j * nx + i, [](int m) { return hm_mrow<MODEL>(m); });
+        if (inside) prefetch_rows<COMB, NM, MODEL>(cb, N, pk + (unsigned)j * nx + i, [](int m) { return hm_mrow<MODEL>(m); });
         if (HAS_Z && c < cend) {
           const unsigned pn = (unsigned)(k + 1) * pstride;
           if (HAS_Y && (TY == 4 || ty < 4)) prefetch_cell(pn + col_yh);
@@ -387,7 +387,7 @@ k_flux_hm(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, size_
         }
         if (inside) {
           const unsigned id = pk + (unsigned)j * nx + i;
-          store_rows<COMB, NM>(L, cb, N, id, Lacc, [](int m) { return hm_mrow<MODEL>(m); });
+          store_rows<COMB, NM, MODEL>(L, cb, N, id, Lacc, [](int m) { return hm_mrow<MODEL>(m); });
         }
       }
     }

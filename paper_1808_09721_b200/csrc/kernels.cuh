@@ -21,6 +21,7 @@ struct StageCoef {
   double a;                // a_ii dt
   double cL[2], cP[2];     // q_ex = qn + cL0 L1 + cL1 L2 + cP0 Psi1 + cP1 Psi2            (a~_ij dt, a_ij dt)
   double hL[2], hP[3];     // A    = qn + hL0 L1 + hL1 L2 + hP0 Psi1 + hP1 Psi2 + hP2 Psi  (w~_j dt, w_j dt)
+  int a_src_only;          // MKA: store A only for the rows with a source (the flux epilogue rebuilds the others, FluxComb.theta)
 };
 
 template <int MODEL> struct ConsRows { const double* r[Dim<MODEL>::NC]; };
@@ -210,7 +211,7 @@ __global__ void __launch_bounds__(128, (NL == 0 && !MKA) ? 5 : 4) k_stage_resist
           if (MKA) av = fma(k.hL[1], l2, av);
           qe[v] = fma(k.cL[1], l2, qe[v]);
         }
-        if (MKA && (v < 8 || v == 11)) A[(size_t)v * N + c] = av;
+        if (MKA && !k.a_src_only && (v < 8 || v == 11)) A[(size_t)v * N + c] = av;
       }
 #pragma unroll
       for (int j = 0; j < R_NS; ++j) {
@@ -326,7 +327,7 @@ __global__ void __launch_bounds__(128) k_stage_two_fluid(const double* __restric
           if (MKA) av = fma(k.hL[1], l2, av);
           qe[v] = fma(k.cL[1], l2, qe[v]);
         }
-        if (MKA && (v < 6 || (v >= 10 && v < 13))) A[(size_t)v * N + c] = av;
+        if (MKA && !k.a_src_only && (v < 6 || (v >= 10 && v < 13))) A[(size_t)v * N + c] = av;
       }
 #pragma unroll
       for (int j = 0; j < T_NS; ++j) {
