@@ -301,12 +301,12 @@ def run_ours(args):
     else:
         roof = {"bound": "hbm", "kernel": dom, "achieved": alg_bytes[dom] / (avg_ms * 1e-3) * 1e-9, "peak": hbm_peak,
                 "unit": "GB/s", "peak_source": peak_src + " (MEASURED_PEAKS.json hbm_gbs)", "traffic": None}
-    # DRAM bytes per launch of that kernel from the committed `ncu --set full` capture (profiles/r1e_kernels.md:
-    # dram__bytes_read.sum + dram__bytes_write.sum; F1 4.589 GB, F2 6.509 GB, S1 4.517, S2 9.498 before A shrank to its 5 source rows, P 2.790), cfg5 / SSP2(222) only
-    ncu_traffic = {"flux": 0.5 * (4.589e9 + 6.509e9), "stage1": 4.517e9, "stage2": 9.498e9, "combine_c2p": 2.790e9}
+    # DRAM bytes per launch of that kernel from the committed `ncu --set full` capture (profiles/r1g_kernels.md:
+    # dram__bytes_read.sum + dram__bytes_write.sum; F1 4.586 GB, F2 6.552 GB, S1 4.526, S2 8.291, P 2.790), cfg5 / SSP2(222) only
+    ncu_traffic = {"flux": 0.5 * (4.586e9 + 6.552e9), "stage1": 4.526e9, "stage2": 8.291e9, "combine_c2p": 2.790e9}
     if args.workload == "cfg5" and nstage == 2 and fused:
         roof["traffic"] = ncu_traffic[dom]
-        roof["traffic_source"] = "ncu --set full, profiles/r1e_kernels.md (per launch; flux = mean of F1 and F2)"
+        roof["traffic_source"] = "ncu --set full, profiles/r1g_kernels.md (per launch; flux = mean of F1 and F2)"
     roof["frac"] = roof["achieved"] / roof["peak"]
     roof["avg_launch_ms"] = avg_ms
     roof["kernel_time_shares"] = shares
