@@ -278,7 +278,8 @@ def run_ours(args):
     nfl = max(kt["flux"]["launches"], 1) / (float(nstage) * args.steps)   # launches per L(q): 1 fused, naxes split
     alg_bytes = {
         "stage1": 34 * 8 * ncell,                                   # R qn 14 + w 5; W E*,psi*,phi* 5 + w 5 + Psi1 5
-        "stage2": 62 * 8 * ncell,                                   # R qn 14 + L1 14 + Psi1 5 + w 5; W q2 14 + w 5 + (A, source rows 5 | Psi2 5)
+        # fused SSP2: F1 has left q_ex of the 9 rows without a source in qs: R q_ex 9 + qn 5 + L1 5 + Psi1 5 + w 5; W q2 5 + w 5 + A 5
+        "stage2": ((44 if nstage == 2 else 62) if fused else 62) * 8 * ncell,   # else R qn 14 + L1 14 + Psi1 5 + w 5; W q2 14 + w 5 + Psi2 5
         "flux": ((33 * (nstage - 1) + 47) / float(nstage) if fused else 33 / nfl) * 8 * ncell,   # F: R 19, W 14; fused last F: R 19 + qn 9 + A 5, W 14
         "combine_c2p": (21 if fused else 76) * 8 * ncell,           # fused: con2prim R 11 + 5, W 5; else k_final R 57, W 19
     }

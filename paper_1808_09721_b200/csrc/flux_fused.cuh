@@ -190,7 +190,10 @@ template <int MODEL> struct FFSmem {
 // theta > 0: for the rows WITHOUT a source the last stage is q_last = qn + c (sum of the earlier L), so their part of eq (11)
 // is A_v = (1 - theta) qn_v + theta q_last,v (SSP2(222): theta = 1/2; SSP3(332): theta = 2/3) and the stage kernel stores A
 // only for the rows with a source; q_last is this launch's own input (qs).
-struct FluxComb { double* q; const double* A; double hdt; const double* qs; double theta; };
+// pre != 0 (the F1 launch of SSP2(222)): no eq-(11) work; the rows without a source are stored as q_ex of stage 2,
+// q[v] = qs[v] + hdt L_v (q: the stage-state buffer, qs: this launch's input rows = qn, hdt = a~_21 dt), so that stage 2
+// neither reads qn, L1 of those rows nor writes them; the rows with a source are stored as L.
+struct FluxComb { double* q; const double* A; double hdt; const double* qs; double theta; int pre; };
 template <int MODEL> __host__ __device__ constexpr bool has_source(int v) {
   return MODEL == 0 ? ((v >= 8 && v <= 10) || v >= 12) : ((v >= 6 && v <= 9) || v >= 13);
 }
@@ -201,6 +204,18 @@ RMHD_DEV void store_rows(double* __restrict__ L, const FluxComb& cb, size_t N, u
 #pragma unroll
     for (int r = 0; r < NR; ++r) (L + (size_t)row(r) * N)[id] = Lacc[r];
   } else {
+    if (cb.pre) {
+      double z[NR];
+#pragma unroll
+      for (int r = 0; r < NR; ++r) z[r] = has_source<MODEL>(row(r)) ? 0.0 : __ldg((cb.qs + (size_t)row(r) * N) + id);
+#pragma unroll
+      for (int r = 0; r < NR; ++r) {
+        const size_t o = (size_t)row(r) * N;
+        if (has_source<MODEL>(row(r))) (L + o)[id] = Lacc[r];
+        else (cb.q + o)[id] = fma(cb.hdt, Lacc[r], z[r]);
+      }
+      return;
+    }
     double x[NR], y[NR];
     const bool mix = cb.theta > 0.0;
 #pragma unroll
@@ -219,6 +234,7 @@ RMHD_DEV void store_rows(double* __restrict__ L, const FluxComb& cb, size_t N, u
 template <bool COMB, int NR, int MODEL, class ROW>
 RMHD_DEV void prefetch_rows(const FluxComb& cb, size_t N, unsigned id, ROW row) {
   if constexpr (COMB) {
+    if (cb.pre) return;
     const bool mix = cb.theta > 0.0;
 #pragma unroll
     for (int r = 0; r < NR; ++r) {

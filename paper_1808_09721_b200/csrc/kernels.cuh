@@ -22,6 +22,8 @@ struct StageCoef {
   double cL[2], cP[2];     // q_ex = qn + cL0 L1 + cL1 L2 + cP0 Psi1 + cP1 Psi2            (a~_ij dt, a_ij dt)
   double hL[2], hP[3];     // A    = qn + hL0 L1 + hL1 L2 + hP0 Psi1 + hP1 Psi2 + hP2 Psi  (w~_j dt, w_j dt)
   int a_src_only;          // MKA: store A only for the rows with a source (the flux epilogue rebuilds the others, FluxComb.theta)
+  int pre;                 // NL = 1: the rows without a source already hold q_ex = qn + cL0 L1 in qs (written by the F1 epilogue,
+                           // FluxComb.pre); they are read from there and neither qn, L1 of those rows is read nor qs rewritten
 };
 
 template <int MODEL> struct ConsRows { const double* r[Dim<MODEL>::NC]; };
@@ -198,10 +200,11 @@ __global__ void __launch_bounds__(128, (NL == 0 && !MKA) ? 5 : 4) k_stage_resist
   if (valid) {
     double qe[R_NC];
 #pragma unroll
-    for (int v = 0; v < R_NC; ++v) qe[v] = qn[(size_t)v * N + c];
+    for (int v = 0; v < R_NC; ++v) qe[v] = (NL == 1 && k.pre && (v < 8 || v == 11)) ? qs[(size_t)v * N + c] : qn[(size_t)v * N + c];
     if (NL >= 1) {
 #pragma unroll
       for (int v = 0; v < R_NC; ++v) {
+        if (NL == 1 && k.pre && (v < 8 || v == 11)) continue;
         double av = qe[v];
         const double l1 = L1[(size_t)v * N + c];
         if (MKA) av = fma(k.hL[0], l1, av);
@@ -220,7 +223,10 @@ __global__ void __launch_bounds__(128, (NL == 0 && !MKA) ? 5 : 4) k_stage_resist
         if (NL >= 2 && k.cP[1] != 0.0) qe[v] = fma(k.cP[1], Ps2[(size_t)j * N + c], qe[v]);
       }
 #pragma unroll
-      for (int v = 0; v < R_NC; ++v) if (v < 8 || v == 11) qs[(size_t)v * N + c] = qe[v];
+      if (!(NL == 1 && k.pre)) {
+#pragma unroll
+        for (int v = 0; v < R_NC; ++v) if (v < 8 || v == 11) qs[(size_t)v * N + c] = qe[v];
+      }
     }
     qpsi = qe[12]; qphi = qe[13];
     r_stage_init(s, qe, w[c], w[N + c], w[2 * N + c], w[3 * N + c], w[4 * N + c], k.a, P.sigma, P);
@@ -314,10 +320,11 @@ __global__ void __launch_bounds__(128) k_stage_two_fluid(const double* __restric
   if (valid) {
     double qe[T_NC], wg[T_NH];
 #pragma unroll
-    for (int v = 0; v < T_NC; ++v) qe[v] = qn[(size_t)v * N + c];
+    for (int v = 0; v < T_NC; ++v) qe[v] = (NL == 1 && k.pre && (v < 6 || (v >= 10 && v < 13))) ? qs[(size_t)v * N + c] : qn[(size_t)v * N + c];
     if (NL >= 1) {
 #pragma unroll
       for (int v = 0; v < T_NC; ++v) {
+        if (NL == 1 && k.pre && (v < 6 || (v >= 10 && v < 13))) continue;
         double av = qe[v];
         const double l1 = L1[(size_t)v * N + c];
         if (MKA) av = fma(k.hL[0], l1, av);
@@ -336,7 +343,10 @@ __global__ void __launch_bounds__(128) k_stage_two_fluid(const double* __restric
         if (NL >= 2 && k.cP[1] != 0.0) qe[v] = fma(k.cP[1], Ps2[(size_t)j * N + c], qe[v]);
       }
 #pragma unroll
-      for (int v = 0; v < T_NC; ++v) if (v < 6 || (v >= 10 && v < 13)) qs[(size_t)v * N + c] = qe[v];
+      if (!(NL == 1 && k.pre)) {
+#pragma unroll
+        for (int v = 0; v < T_NC; ++v) if (v < 6 || (v >= 10 && v < 13)) qs[(size_t)v * N + c] = qe[v];
+      }
     }
     qpsi = qe[16]; qphi = qe[17];
 #pragma unroll

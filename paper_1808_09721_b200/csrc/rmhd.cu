@@ -43,6 +43,7 @@ struct rmhd_ctx {
   int hm_ty;         // tile rows of the two-role flux kernel: 8 (one 16-warp CTA per SM; default when ny >= 8) or 4 (two CTAs); RMHD_HM_TY
   bool march2d;      // resistive 2-D grids through the marching two-role kernel (default); RMHD_FLUX2D=tile keeps one plane per CTA
   bool comb_mix;     // rows without a source: A rebuilt in the flux epilogue from qn and the last stage state; RMHD_COMBINE=full stores all of A
+  bool pre_s2;       // SSP2 fused path: F1 stores q_ex of stage 2 for the rows without a source; RMHD_PRE=0 disables
   bool one_role;     // RMHD_FLUX=fused1: resistive model through the one-thread-per-column kernel (flux_fused.cuh) instead of flux_hm.cuh
   int sm_count;
   std::vector<EvRec> pending;
@@ -246,7 +247,7 @@ int launch_flux(rmhd_ctx* c, const double* qa, const double* qb, bool mix, const
   if (mix) for (int k = 0; k < NS; ++k) { int v = MODEL == 0 ? (k < 3 ? 8 + k : 9 + k) : (k < 4 ? 6 + k : 9 + k); qr.r[v] = qb + (size_t)v * c->N; }
   for (int v = 0; v < NH; ++v) wr.r[v] = w + (size_t)v * c->N;
   if (uses_fused_flux(c)) {
-    const FluxComb none = {nullptr, nullptr, 0.0, nullptr, 0.0};
+    const FluxComb none = {nullptr, nullptr, 0.0, nullptr, 0.0, 0};
     if constexpr (MODEL == 0) {
       if (c->n[2] == 1 && c->march2d && !c->one_role) return cb ? launch_flux_march2d<true>(c, qr, wr, L, *cb) : launch_flux_march2d<false>(c, qr, wr, L, none);
     }
@@ -289,9 +290,15 @@ int step_once(rmhd_ctx* c) {
   StageCoef k1 = {};
   k1.a = g * dt;
   if ((rc = launch_stage<MODEL, 0, false>(c, KC_STAGE1, k1, c->Ps1, nullptr))) return rc;
-  if ((rc = launch_flux<MODEL>(c, c->q, c->qs, true, c->w, c->L1))) return rc;
   const bool fuse_c = uses_fused_flux(c) && c->fuse_combine;
+  // F1 on the fused path also leaves q_ex of stage 2 for the rows without a source (qn + dt L1) in the stage-state buffer
+  const bool pre = fuse_c && c->comb_mix && c->pre_s2;
+  if (pre) {
+    const FluxComb cb1 = {c->qs, nullptr, dt, c->q, 0.0, 1};
+    if ((rc = launch_flux<MODEL>(c, c->q, c->qs, true, c->w, c->L1, &cb1))) return rc;
+  } else if ((rc = launch_flux<MODEL>(c, c->q, c->qs, true, c->w, c->L1))) return rc;
   StageCoef k2 = {};
+  k2.pre = pre;
   k2.a = g * dt; k2.cL[0] = dt; k2.cP[0] = (1.0 - 2.0 * g) * dt;
   k2.hL[0] = 0.5 * dt; k2.hP[0] = 0.5 * dt; k2.hP[2] = 0.5 * dt;
   if (fuse_c) {
@@ -299,7 +306,7 @@ int step_once(rmhd_ctx* c) {
     // (q^{n+1} = A + dt/2 L2 row by row in the flux kernel's epilogue), then P
     k2.a_src_only = c->comb_mix;
     if ((rc = launch_stage<MODEL, 1, true>(c, KC_STAGE2, k2, nullptr, c->L2))) return rc;
-    const FluxComb cb = {c->q, c->L2, 0.5 * dt, c->qs, c->comb_mix ? 0.5 : 0.0};
+    const FluxComb cb = {c->q, c->L2, 0.5 * dt, c->qs, c->comb_mix ? 0.5 : 0.0, 0};
     if ((rc = launch_flux<MODEL>(c, c->qs, nullptr, false, c->w, c->L2, &cb))) return rc;
     return launch_con2prim<MODEL>(c);
   }
@@ -338,7 +345,7 @@ int step_once_ssp3(rmhd_ctx* c) {
   if ((rc = launch_stage<MODEL, 2, true>(c, KC_STAGE2, k3, nullptr, c->A))) return rc;
   const double wl = 2.0 * dt / 3.0;
   if (fuse3) {
-    const FluxComb cb = {c->q, c->A, wl, c->qs, c->comb_mix ? 2.0 / 3.0 : 0.0};
+    const FluxComb cb = {c->q, c->A, wl, c->qs, c->comb_mix ? 2.0 / 3.0 : 0.0, 0};
     if ((rc = launch_flux<MODEL>(c, c->qs, nullptr, false, c->w, c->L1, &cb))) return rc;
     return launch_con2prim<MODEL>(c);
   }
@@ -408,6 +415,7 @@ int rmhd_create(const rmhd_params* p, rmhd_ctx** out) {
   { const char* e = getenv("RMHD_FLUX"); c->one_role = e && strcmp(e, "fused1") == 0; }
   { const char* e = getenv("RMHD_COMBINE"); c->fuse_combine = !(e && strcmp(e, "split") == 0); }
   { const char* e = getenv("RMHD_COMBINE"); c->comb_mix = !(e && strcmp(e, "full") == 0); }
+  { const char* e = getenv("RMHD_PRE"); c->pre_s2 = !(e && strcmp(e, "0") == 0); }
   { const char* e = getenv("RMHD_FLUX2D"); c->march2d = !(e && strcmp(e, "tile") == 0); }
   { const char* e = getenv("RMHD_HM_TY"); c->hm_ty = e ? (atoi(e) == 8 ? 8 : 4) : (p->ny >= 8 ? 8 : 4); }
   c->sm_count = 148;
