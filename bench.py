@@ -303,8 +303,8 @@ def run_ours(args):
         roof = {"bound": "hbm", "kernel": dom, "achieved": alg_bytes[dom] / (avg_ms * 1e-3) * 1e-9, "peak": hbm_peak,
                 "unit": "GB/s", "peak_source": peak_src + " (MEASURED_PEAKS.json hbm_gbs)", "traffic": None}
     # DRAM bytes per launch of that kernel from the committed `ncu --set full` capture (profiles/r1g_kernels.md:
-    # dram__bytes_read.sum + dram__bytes_write.sum; F1 4.586 GB, F2 6.552 GB, S1 4.526, S2 8.291, P 2.790), cfg5 / SSP2(222) only
-    ncu_traffic = {"flux": 0.5 * (4.586e9 + 6.552e9), "stage1": 4.526e9, "stage2": 8.291e9, "combine_c2p": 2.790e9}
+    # dram__bytes_read.sum + dram__bytes_write.sum; F1 4.589 GB, F2 6.484 GB, S1 4.526, S2 5.873, P 2.790), cfg5 / SSP2(222) only
+    ncu_traffic = {"flux": 0.5 * (4.589e9 + 6.484e9), "stage1": 4.526e9, "stage2": 5.873e9, "combine_c2p": 2.790e9}
     if args.workload == "cfg5" and nstage == 2 and fused:
         roof["traffic"] = ncu_traffic[dom]
         roof["traffic_source"] = "ncu --set full, profiles/r1g_kernels.md (per launch; flux = mean of F1 and F2)"
