@@ -308,6 +308,8 @@ def run_ours(args):
     if args.workload == "cfg5" and nstage == 2 and fused:
         roof["traffic"] = ncu_traffic[dom]
         roof["traffic_source"] = "ncu --set full, profiles/r1g_kernels.md (per launch; flux = mean of F1 and F2)"
+        if dom == "flux":   # sm__inst_executed_pipe_fp64 pct of peak, mean of F1 (44.8) and F2 (43.0): the instruction-issue view of the same roofline
+            roof["fp64_pipe_busy_ncu"] = 0.439
     roof["frac"] = roof["achieved"] / roof["peak"]
     roof["avg_launch_ms"] = avg_ms
     roof["kernel_time_shares"] = shares
