@@ -185,7 +185,7 @@ __global__ void __launch_bounds__(256) k_con2prim(const double* __restrict__ con
 // that the last flux launch finishes the step with q^{n+1}_v = A_v + w~_last dt L_last,v (flux_fused.cuh, FluxComb).
 // =======================================================================================
 template <int NL, bool MKA = false>
-__global__ void __launch_bounds__(128, NL <= 1 ? 5 : 4) k_stage_resistive(const double* __restrict__ qn, const double* __restrict__ L1,
+__global__ void __launch_bounds__(128, 5) k_stage_resistive(const double* __restrict__ qn, const double* __restrict__ L1,
                                                          const double* __restrict__ L2, const double* __restrict__ Ps1,
                                                          const double* __restrict__ Ps2, double* __restrict__ w,
                                                          double* __restrict__ qs, double* __restrict__ Ps, double* __restrict__ A,
