@@ -11,6 +11,7 @@
 #include "kernels.cuh"
 #include "flux_fused.cuh"
 #include "flux_hm.cuh"
+#include "flux_vp.cuh"
 
 using namespace rmhd;
 
@@ -46,6 +47,8 @@ struct rmhd_ctx {
   bool pre_s2;       // SSP2 fused path: F1 stores q_ex of stage 2 for the rows without a source; RMHD_PRE=0 disables
   bool one_role;     // RMHD_FLUX=fused1: resistive model through the one-thread-per-column kernel (flux_fused.cuh) instead of flux_hm.cuh
   int sm_count;
+  bool vp_ok;        // 3-D resistive grids with even nx: the TMA-staged, variable-specialised flux kernel (flux_vp.cuh)
+  CUtensorMap tmap;  // 4-D view (x, y, z, row) of the whole state allocation, box = one haloed tile plane of one row
   std::vector<EvRec> pending;
   std::vector<cudaEvent_t> ev_pool;
   double ms[KC_N];
@@ -236,6 +239,62 @@ int launch_flux_march2d(rmhd_ctx* c, const ConsRows<0>& qr, const HydRows<0>& wr
   return RMHD_OK;
 }
 
+// 3-D grids, resistive model: TMA-staged planes, one warp per row with a non-trivial flux (flux_vp.cuh)
+template <int MODE>
+int launch_flux_vp(rmhd_ctx* c, const ConsRows<0>& qr, const HydRows<0>& wr, double* L, const FluxComb& cb) {
+  using GM = VPGeom<0>;
+  using FS = FSet<0>;
+  static bool attr_set[8] = {false, false, false, false, false, false, false, false};
+  const int nx = c->n[0], ny = c->n[1], nz = c->n[2];
+  const size_t smem = GM::bytes();
+  if (!attr_set[c->device & 7]) {
+    CK(c, cudaFuncSetAttribute(k_flux_vp<MODE, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    attr_set[c->device & 7] = true;
+  }
+  VPRows<0> rows;
+  auto row_of = [&](const double* p) { return (int)((size_t)(p - c->q) / c->N); };
+  for (int h = 0; h < GM::NHV; ++h) rows.h[h] = row_of(qr.r[FS::hv(h)]);
+  for (int v = 0; v < GM::NH; ++v) rows.h[GM::NHV + v] = row_of(wr.r[v]);
+  for (int m = 0; m < 8; ++m) rows.m[m] = row_of(qr.r[hm_mrow<0>(m)]);
+  const int gx = (nx + VP_TX - 1) / VP_TX, gy = (ny + VP_TY - 1) / VP_TY;
+  // z segments: the count (segments of >= 16 planes) that wastes least, counting the partially filled last wave of CTAs
+  // (one per SM) and the 4 feed-only planes of every segment
+  int nseg = 1, seg_len = nz;
+  {
+    const long long tiles = (long long)gx * gy, slots = c->sm_count;
+    double best = 1e300;
+    for (int s = 1; s <= (nz + 15) / 16 && s <= 64; ++s) {
+      const int len = (nz + s - 1) / s, cnt = (nz + len - 1) / len;
+      const long long ctas = tiles * cnt, waves = (ctas + slots - 1) / slots;
+      const double cost = (double)waves * slots / (double)ctas * (1.0 + 3.0 / len);
+      if (cost < best - 1e-9) { best = cost; nseg = cnt; seg_len = len; }
+    }
+  }
+  dim3 grid(gx, gy, nseg);
+  Timed t(c, KC_FLUX);
+  k_flux_vp<MODE, 0><<<grid, GM::THREADS, smem, c->stream>>>(c->tmap, rows, qr, wr, L, c->N, nx, ny, nz, c->p.bc[0], c->p.bc[1], c->p.bc[2],
+                                                            0.5 / c->dx[0], 0.5 / c->dx[1], 0.5 / c->dx[2], seg_len, c->P, cb);
+  CK(c, cudaGetLastError());
+  return RMHD_OK;
+}
+
+// tensor map of the state allocation for flux_vp.cuh (driver entry point through the runtime: no -lcuda)
+int make_tensor_map(rmhd_ctx* c, size_t rows) {
+  typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                               const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  CK(c, cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+  if (!fn || qres != cudaDriverEntryPointSuccess) { c->err = "cuTensorMapEncodeTiled not available"; return RMHD_ERR_CUDA; }
+  const cuuint64_t dims[4] = {(cuuint64_t)c->n[0], (cuuint64_t)c->n[1], (cuuint64_t)c->n[2], (cuuint64_t)rows};
+  const cuuint64_t strides[3] = {sizeof(double) * (cuuint64_t)c->n[0], sizeof(double) * (cuuint64_t)c->n[0] * c->n[1], sizeof(double) * (cuuint64_t)c->N};
+  const cuuint32_t box[4] = {VP_XW, VP_YR, 1, 1}, est[4] = {1, 1, 1, 1};
+  const CUresult r = ((EncodeFn)fn)(&c->tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->q, dims, strides, box, est, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                    CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { char b[96]; snprintf(b, sizeof b, "cuTensorMapEncodeTiled failed (%d)", (int)r); c->err = b; return RMHD_ERR_CUDA; }
+  return RMHD_OK;
+}
+
 inline bool uses_fused_flux(const rmhd_ctx* c) { return c->fused_flux && c->n[0] > 1 && c->n[1] > 1; }
 
 // `cb` (fused path only): store the eq-(11) update of q instead of L (a5 fused into F2)
@@ -249,6 +308,11 @@ int launch_flux(rmhd_ctx* c, const double* qa, const double* qb, bool mix, const
   if (uses_fused_flux(c)) {
     const FluxComb none = {nullptr, nullptr, 0.0, nullptr, 0.0, 0};
     if constexpr (MODEL == 0) {
+      if (c->vp_ok) {
+        if (!cb) return launch_flux_vp<0>(c, qr, wr, L, none);
+        if (cb->pre) return launch_flux_vp<1>(c, qr, wr, L, *cb);
+        if (cb->theta > 0.0) return launch_flux_vp<2>(c, qr, wr, L, *cb);
+      }
       if (c->n[2] == 1 && c->march2d && !c->one_role) return cb ? launch_flux_march2d<true>(c, qr, wr, L, *cb) : launch_flux_march2d<false>(c, qr, wr, L, none);
     }
     if (cb) return c->n[2] > 1 ? launch_flux_fused<MODEL, true, true>(c, qr, wr, L, *cb) : launch_flux_fused<MODEL, false, true>(c, qr, wr, L, *cb);
@@ -436,6 +500,15 @@ int rmhd_create(const rmhd_params* p, rmhd_ctx** out) {
   b += (size_t)c->nh * c->N; c->Ps1 = b;
   b += (size_t)c->ns * c->N; c->Ps2 = b;
   if (p->integrator == RMHD_SSP3_332) { b += (size_t)c->ns * c->N; c->A = b; }
+  c->vp_ok = false;
+  {
+    const char* ev = getenv("RMHD_FLUX");
+    const bool want = !(ev && (strcmp(ev, "hm") == 0 || strcmp(ev, "split") == 0 || strcmp(ev, "fused1") == 0));
+    if (want && p->model == RMHD_RESISTIVE && p->nx > 1 && p->ny > 1 && p->nz > 1 && p->nx % 2 == 0) {
+      if (make_tensor_map(c, rows)) { g_create_error = c->err; rmhd_destroy(c); return RMHD_ERR_CUDA; }
+      c->vp_ok = true;
+    }
+  }
   e = cudaMemsetAsync(c->q, 0, sizeof(double) * rows * c->N, c->stream);
   if (e != cudaSuccess) { fail_cuda(nullptr, e, "clearing device state"); rmhd_destroy(c); return RMHD_ERR_CUDA; }
   if (reset_stats(c)) { g_create_error = c->err; rmhd_destroy(c); return RMHD_ERR_CUDA; }

@@ -193,6 +193,9 @@ def _random_state(model, shape, seed):
     (0, (1, 1, 67), (0, 0, 0)), (0, (1, 1, 130), (1, 1, 1)), (0, (1, 9, 70), (1, 0, 0)), (0, (1, 33, 5), (0, 1, 0)),
     (0, (7, 10, 35), (0, 1, 0)), (0, (11, 3, 66), (1, 0, 1)), (0, (9, 1, 40), (0, 0, 1)),
     (0, (37, 6, 33), (1, 1, 1)), (0, (50, 5, 40), (0, 0, 0)), (0, (2, 2, 2), (1, 0, 1)), (1, (35, 6, 33), (0, 1, 1)),
+    # even nx, 3-D, resistive: the TMA-staged kernel (flux_vp.cuh); partial tiles in x and y, several z segments, both BCs
+    (0, (7, 10, 34), (0, 1, 0)), (0, (20, 19, 70), (1, 0, 1)), (0, (5, 8, 32), (0, 0, 0)), (0, (40, 16, 64), (1, 1, 1)),
+    (0, (3, 2, 4), (1, 1, 0)), (0, (33, 9, 30), (0, 0, 1)),
     (1, (1, 1, 67), (1, 0, 0)), (1, (1, 12, 37), (0, 1, 0)), (1, (6, 9, 34), (1, 1, 0)),
 ])
 def test_flux_divergence_parity(B, O, model, shape, bc):
