@@ -44,7 +44,8 @@ template <int MODEL> struct VPGeom {
   static constexpr int GX = 2 * NHV * VP_TY * VP_XW, GY = 2 * NHV * VP_YR * VP_TX, GZ = 2 * NHV * VP_TY * VP_TX;
   static constexpr int FX = NHV * VP_TY;                                       // right face of tile column 31, hydro rows
   static constexpr int NBAR = 5;                                               // mbarriers (8 bytes each), after the arrays
-  static constexpr size_t bytes() { return sizeof(double) * (RAWH + 2 * RAWM + GX + GY + 3 * GZ + FX + NBAR); }
+  static constexpr int NTAB = NRH + NRM;                                       // row pointers of the staged planes
+  static constexpr size_t bytes() { return sizeof(double) * (RAWH + 2 * RAWM + GX + GY + 3 * GZ + FX + NBAR + NTAB); }
   static constexpr unsigned TXH = sizeof(double) * RAWH, TXM = sizeof(double) * RAWM;
 };
 
@@ -88,6 +89,38 @@ RMHD_DEV double weno_ds(double b, double d0, double d1, double S0, double S1) {
   const double r = fma(r0, fma(er, er, er), r0);
   return fma(0.5, fma(S1 * r, d0 - d1, d1), b);
 }
+// G independent cell pairs / reconstructions in OPERATION-MAJOR order: ptxas keeps the source order of independent
+// chains, and the FP64 pipe needs >= 4 instructions in flight per SM sub-partition (8-cycle dependent latency, one
+// issue per 2 cycles)
+template <int G> RMHD_DEV void pair_terms_batch(const double* ul, const double* ur, double* d, double* S) {
+#pragma unroll
+  for (int g = 0; g < G; ++g) d[g] = ur[g] - ul[g];
+#pragma unroll
+  for (int g = 0; g < G; ++g) S[g] = fma(d[g], d[g], VP_EPS);
+#pragma unroll
+  for (int g = 0; g < G; ++g) S[g] = S[g] * S[g];
+}
+template <int G> RMHD_DEV void weno_ds_batch(const double* b, const double* d0, const double* d1, const double* S0, const double* S1, double* out) {
+  double den[G], r0[G], er[G];
+#pragma unroll
+  for (int g = 0; g < G; ++g) den[g] = fma(0.5, S0[g], S1[g]);
+#pragma unroll
+  for (int g = 0; g < G; ++g) r0[g] = rcp_seed(den[g]);
+#pragma unroll
+  for (int g = 0; g < G; ++g) er[g] = fma(-den[g], r0[g], 1.0);
+#pragma unroll
+  for (int g = 0; g < G; ++g) er[g] = fma(er[g], er[g], er[g]);
+#pragma unroll
+  for (int g = 0; g < G; ++g) r0[g] = fma(r0[g], er[g], r0[g]);
+#pragma unroll
+  for (int g = 0; g < G; ++g) r0[g] = S1[g] * r0[g];
+#pragma unroll
+  for (int g = 0; g < G; ++g) den[g] = d0[g] - d1[g];
+#pragma unroll
+  for (int g = 0; g < G; ++g) den[g] = fma(r0[g], den[g], d1[g]);
+#pragma unroll
+  for (int g = 0; g < G; ++g) out[g] = fma(0.5, den[g], b[g]);
+}
 // value at the face between b and c biased to a (physics.cuh weno3 on unscaled fields)
 RMHD_DEV double weno_u(double a, double b, double c) {
   double d0, S0, d1, S1;
@@ -97,17 +130,25 @@ RMHD_DEV double weno_u(double a, double b, double c) {
 }
 
 // store one row of one cell (element e = row * N + id): L itself, or the q_ex / eq-(11) update (FluxComb, flux_fused.cuh)
+// split in two so that the loads are issued before the reconstructions of the cell and used after them
 template <int MODE>
-RMHD_DEV void store_row(double* __restrict__ L, const FluxComb& cb, size_t e, bool src, double val) {
+RMHD_DEV void epi_load(const FluxComb& cb, size_t e, bool src, double& x, double& y) {
+  x = y = 0.0;
+  if constexpr (MODE == 1) { if (!src) x = __ldg(cb.qs + e); }
+  if constexpr (MODE == 2) {
+    if (src) x = __ldg(cb.A + e);
+    else { x = cb.q[e]; y = __ldg(cb.qs + e); }
+  }
+}
+template <int MODE>
+RMHD_DEV void store_row(double* __restrict__ L, const FluxComb& cb, size_t e, bool src, double val, double x, double y) {
   if constexpr (MODE == 0) {
     L[e] = val;
   } else if constexpr (MODE == 1) {
     if (src) L[e] = val;
-    else cb.q[e] = fma(cb.hdt, val, __ldg(cb.qs + e));
+    else cb.q[e] = fma(cb.hdt, val, x);
   } else {
-    double a;
-    if (src) a = __ldg(cb.A + e);
-    else { const double x = cb.q[e], y = __ldg(cb.qs + e); a = fma(cb.theta, y - x, x); }
+    const double a = src ? x : fma(cb.theta, y - x, x);
     cb.q[e] = fma(cb.hdt, val, a);
   }
 }
@@ -140,16 +181,22 @@ RMHD_DEV double shfl_idx(double v, int src) {
   return __hiloint2double(hi, lo);
 }
 
+#ifdef VP_TRACE
+__device__ long long vp_trace_buf[16 * 80 * 8];
+#define VP_T(slot) do { if (lane == 0 && blockIdx.x == 2 && blockIdx.y == 5 && blockIdx.z == 1 && c - k0 + 2 < 80) vp_trace_buf[(wrp * 80 + (c - k0 + 2)) * 8 + (slot)] = clock64(); } while (0)
+#else
+#define VP_T(slot)
+#endif
+
 struct VPTile { int i0, j0, nL, xR0, nOx, nT, yB0, nOy; };
 
 // virtual ghost zones (a6) of a staged plane: the elements of the box outside the grid (halo of boundary CTAs, tail of a
 // partial tile) are replaced by their outflow / periodic image, read from global memory.  One copy, called by every thread.
 template <int MODEL>
-__device__ __noinline__ void vp_fixup(double* rawH, double* rM, const ConsRows<MODEL>& qin, const HydRows<MODEL>& win, const VPTile& T,
+__device__ __noinline__ void vp_fixup(double* rawH, double* rM, const double* const* tab, const VPTile& T,
                                       int kz, int nx, int ny, int bcx, int bcy, int nthreads) {
-  using FS = FSet<MODEL>;
-  constexpr int NHV = FS::NHV, NRH = VPGeom<MODEL>::NRH, XW = VP_XW, YR = VP_YR, PL = VP_PL;
-  auto src = [&](int v) -> const double* { return v < NHV ? qin.r[FS::hv(v)] : (v < NRH ? win.r[v - NHV] : qin.r[hm_mrow<MODEL>(v - NRH)]); };
+  constexpr int NRH = VPGeom<MODEL>::NRH, XW = VP_XW, YR = VP_YR, PL = VP_PL;
+  auto src = [&](int v) -> const double* { return tab[v]; };
   const unsigned pz = (unsigned)kz * ny;
   for (int it = threadIdx.x; it < (NRH + 8) * YR * T.nOx; it += nthreads) {          // out-of-range columns, every row of the box
     const int rw = it / T.nOx, o = it - rw * T.nOx, v = rw / YR, y = rw - v * YR;
@@ -186,9 +233,11 @@ k_flux_vp(const __grid_constant__ CUtensorMap tmap, VPRows<MODEL> rows, ConsRows
   double* fX = gZ + 3 * GM::GZ;
   unsigned long long* bars = (unsigned long long*)(fX + GM::FX);
   unsigned long long &fullH = bars[0], *fullM = bars + 1, *doneM = bars + 3;
+  const double** tab = (const double**)(bars + GM::NBAR);   // staged rows: NHV cons rows, NH primitives, B, E, psi, phi
   const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
-  const bool is_mx = wrp >= WH && wrp < WH + WM;
-  const bool issuer = tid == 32 * (WH + WM);             // lane 0 of the first helper warp
+  // warp roles: Maxwell 0 .. WM-1, helpers WM .. WM+WX-1, hydro WM+WX .. (the scheduler favours high warp ids: the hydro
+  // warps, whose phases are chained by the barriers, go first; the decoupled Maxwell warps fill the gaps)
+  const bool is_mx = wrp < WM;
   VPTile T;
   T.i0 = blockIdx.x * TX; T.j0 = blockIdx.y * TY;
   // elements of the staged box that fall outside the grid
@@ -201,6 +250,12 @@ k_flux_vp(const __grid_constant__ CUtensorMap tmap, VPRows<MODEL> rows, ConsRows
 
   if (tid == 0) {
     if (smem_u32(sm) & 127u) __trap();
+#pragma unroll
+    for (int v = 0; v < NHV; ++v) tab[v] = qin.r[FS::hv(v)];
+#pragma unroll
+    for (int v = 0; v < NH; ++v) tab[NHV + v] = win.r[v];
+#pragma unroll
+    for (int m = 0; m < 8; ++m) tab[NRH + m] = qin.r[hm_mrow<MODEL>(m)];
     mbar_init(&fullH, 1); mbar_init(&fullM[0], 1); mbar_init(&fullM[1], 1);
     mbar_init(&doneM[0], WM * 32); mbar_init(&doneM[1], WM * 32);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -208,20 +263,23 @@ k_flux_vp(const __grid_constant__ CUtensorMap tmap, VPRows<MODEL> rows, ConsRows
   __syncthreads();
 
   // staged step t (c = k0 + t): plane bc(k0 + t - 2) of the hydro rows / of the Maxwell rows (buffer t & 1)
+  // (called by the whole first helper warp: lane 0 arms the barrier, then one lane per row issues its box)
+  const int my_row = lane < NRH ? rows.h[lane < NRH ? lane : 0] : rows.m[(lane - NRH) & 7];
   auto issue_H = [&](int t) {
     const int kz = bc1(k0 + t - 2, nz, bcz);
-    mbar_expect_tx(&fullH, GM::TXH);
-#pragma unroll 1
-    for (int v = 0; v < NRH; ++v) tma_load_plane(rawH + v * PL, &tmap, i0 - 2, j0 - 2, kz, rows.h[v], &fullH);
+    if (lane == 0) mbar_expect_tx(&fullH, GM::TXH);
+    __syncwarp();
+    if (lane < NRH) tma_load_plane(rawH + lane * PL, &tmap, i0 - 2, j0 - 2, kz, my_row, &fullH);
   };
   auto issue_M = [&](int t) {
     const int kz = bc1(k0 + t - 2, nz, bcz);
     double* dst = rawM + (t & 1) * GM::RAWM;
-    mbar_expect_tx(&fullM[t & 1], GM::TXM);
-#pragma unroll 1
-    for (int v = 0; v < 8; ++v) tma_load_plane(dst + v * PL, &tmap, i0 - 2, j0 - 2, kz, rows.m[v], &fullM[t & 1]);
+    if (lane == 0) mbar_expect_tx(&fullM[t & 1], GM::TXM);
+    __syncwarp();
+    if (lane >= NRH && lane < NRH + 8) tma_load_plane(dst + (lane - NRH) * PL, &tmap, i0 - 2, j0 - 2, kz, my_row, &fullM[t & 1]);
   };
   const int tmax = k1 + 1 - k0;              // staged steps t = 0 .. tmax
+  const bool issuer = wrp == WM;             // the first helper warp
   if (issuer) { issue_H(0); issue_M(0); }
 
   const int i = i0 + lane;
@@ -229,8 +287,9 @@ k_flux_vp(const __grid_constant__ CUtensorMap tmap, VPRows<MODEL> rows, ConsRows
 
   if (!is_mx) {
     // ======================================= hydro and helper warps =======================================
-    const int pw = wrp < WH ? wrp : wrp - WM;            // 0 .. WH + WX - 1: phase-A warp
-    const int h = wrp < WH ? wrp : 0, row = FS::hv(h);
+    const bool is_hyd = wrp >= WM + WX;
+    const int h = is_hyd ? wrp - WM - WX : 0, row = FS::hv(h);
+    const int pw = is_hyd ? h : WH + wrp - WM;           // 0 .. WH + WX - 1: phase-A warp
     const bool rsrc = has_source<MODEL>(row);
     const size_t erow = (size_t)row * N;
     double pend[TY], Gprev[TY];                          // z carry of row hv(h) for the TY cells of this column
@@ -245,39 +304,37 @@ k_flux_vp(const __grid_constant__ CUtensorMap tmap, VPRows<MODEL> rows, ConsRows
       const int k = c - 2, t = c - k0;
       const bool staged = t >= 0, do_xy = c >= k0 + 2;
       double* rM = rawM + (t & 1) * GM::RAWM;
+      // z feed: plane c, own row pw, straight from global memory (L2: prefetched by the helper warps one step earlier);
+      // issued first, used after the x / y fields
+      double zq[NC], zw[NH];
+      VP_T(0);
+      {
+        const unsigned id = (unsigned)bc1(c, nz, bcz) * pstride + (unsigned)jrow * nx + im;
+#pragma unroll
+        for (int hh = 0; hh < NHV; ++hh) zq[FS::hv(hh)] = __ldg(qin.r[FS::hv(hh)] + id);
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { zq[FS::IB + d] = __ldg(qin.r[FS::IB + d] + id); zq[FS::IE + d] = __ldg(qin.r[FS::IE + d] + id); }
+#pragma unroll
+        for (int v = 0; v < NH; ++v) zw[v] = __ldg(win.r[v] + id);
+      }
       if (staged) {
         if (issuer && t + 1 <= tmax) {        // Maxwell plane of the next step into the other buffer, once its readers are done
-          if (t >= 1) mbar_wait_par(&doneM[(t + 1) & 1], ((t - 1) >> 1) & 1);
+          if (t >= 1 && lane == 0) mbar_wait_par(&doneM[(t + 1) & 1], ((t - 1) >> 1) & 1);
+          __syncwarp();
           issue_M(t + 1);
         }
         mbar_wait_par(&fullH, t & 1);
         mbar_wait_par(&fullM[t & 1], (t >> 1) & 1);
         if (boundary) {
-          vp_fixup<MODEL>(rawH, rM, qin, win, T, bc1(k, nz, bcz), nx, ny, bcx, bcy, NT);
+          vp_fixup<MODEL>(rawH, rM, tab, T, bc1(k, nz, bcz), nx, ny, bcx, bcy, NT);
           vp_bar<0, NT>();
         }
       }
+      VP_T(1);
       // ---------------- phase A: fields g+- = f +- q of the hydro rows ----------------
       {
         double q_[NC], w_[NH], fh[NHV];
         Com<MODEL> cm;
-        {   // z fields of plane c, own row pw, from global memory -> ring slot c mod 3
-          const unsigned id = (unsigned)bc1(c, nz, bcz) * pstride + (unsigned)jrow * nx + im;
-#pragma unroll
-          for (int hh = 0; hh < NHV; ++hh) q_[FS::hv(hh)] = __ldg(qin.r[FS::hv(hh)] + id);
-#pragma unroll
-          for (int d = 0; d < 3; ++d) { q_[FS::IB + d] = __ldg(qin.r[FS::IB + d] + id); q_[FS::IE + d] = __ldg(qin.r[FS::IE + d] + id); }
-#pragma unroll
-          for (int v = 0; v < NH; ++v) w_[v] = __ldg(win.r[v] + id);
-          cell_common(q_, w_, P, cm);
-          cell_hflux<2>(q_, w_, cm, P, fh);
-          double* gz = gZ + ((c + 3) % 3) * GM::GZ + pw * TX + lane;
-#pragma unroll
-          for (int hh = 0; hh < NHV; ++hh) {
-            gz[hh * TY * TX] = fh[hh] + q_[FS::hv(hh)];
-            gz[(NHV + hh) * TY * TX] = fh[hh] - q_[FS::hv(hh)];
-          }
-        }
         if (staged) {
           // x / y fields of plane k from the staged box: own row, then this warp's halo task
 #pragma unroll 1
@@ -314,23 +371,35 @@ k_flux_vp(const __grid_constant__ CUtensorMap tmap, VPRows<MODEL> rows, ConsRows
             }
           }
         }
+        VP_T(2);
+        {   // z fields of plane c -> ring slot c mod 3
+          cell_common(zq, zw, P, cm);
+          cell_hflux<2>(zq, zw, cm, P, fh);
+          double* gz = gZ + ((c + 3) % 3) * GM::GZ + pw * TX + lane;
+#pragma unroll
+          for (int hh = 0; hh < NHV; ++hh) {
+            gz[hh * TY * TX] = fh[hh] + zq[FS::hv(hh)];
+            gz[(NHV + hh) * TY * TX] = fh[hh] - zq[FS::hv(hh)];
+          }
+        }
       }
+      VP_T(3);
       vp_bar<1, NPA>();                                       // S1: fields of this step are in shared memory
+      VP_T(4);
       if (issuer && staged && t + 1 <= tmax) issue_H(t + 1);  // the hydro buffer is free: next plane
 
-      if (wrp >= WH) {
+      if (!is_hyd) {
         // helper warps: L2 prefetch of what the next step reads from global memory (z feed plane c+1; epilogue rows of plane k+1)
         if (c + 1 <= k1 + 1) {
           const unsigned pc = (unsigned)bc1(c + 1, nz, bcz) * pstride + (unsigned)i0;
           const unsigned pk1 = (unsigned)min(k + 1, nz - 1) * pstride + (unsigned)i0;
-          for (int it = (wrp - WH - WM) * 32 + lane; it < 2 * TY * (NC + NH + NC); it += 32 * WX) {
-            const int half = it & 1, r = (it >> 1) & (TY - 1), v = it >> 4;      // TY = 8
+          for (int it = (wrp - WM) * 32 + lane; it < 2 * TY * (GM::NTAB + NC); it += 32 * WX) {
+            const int half = it & 1, r = (it >> 1) & (TY - 1), v = it >> 4;      // TY = 8: one 128-byte line per item
             const unsigned col = (unsigned)bc1(j0 + r, ny, bcy) * nx + 16 * half;
             if (i0 + 16 * half >= nx) continue;
-            if (v < NC) prefetch_l2(qin.r[v] + pc + col);
-            else if (v < NC + NH) prefetch_l2(win.r[v - NC] + pc + col);
+            if (v < GM::NTAB) prefetch_l2(tab[v] + pc + col);
             else if (MODE != 0 && k + 1 >= k0 && k + 1 < k1) {
-              const int vr = v - NC - NH;
+              const int vr = v - GM::NTAB;
               const size_t e = (size_t)vr * N + pk1 + col;
               if (MODE == 1) { if (!has_source<MODEL>(vr)) prefetch_l2(cb.qs + e); }
               else prefetch_l2((has_source<MODEL>(vr) ? cb.A : (const double*)cb.q) + e);
@@ -346,6 +415,14 @@ k_flux_vp(const __grid_constant__ CUtensorMap tmap, VPRows<MODEL> rows, ConsRows
         const double* zn = gZ + ((c + 3) % 3) * GM::GZ + lane;      // plane c
         const double* zm = gZ + ((c + 2) % 3) * GM::GZ + lane;      // plane c-1
         const double* zo = gZ + ((c + 1) % 3) * GM::GZ + lane;      // plane c-2
+        // operands of the q_ex / eq-(11) epilogue of the TY cells: issued now, used at the stores
+        const size_t ebase = erow + (unsigned)k * pstride + (unsigned)j0 * nx + i;
+        double ex[TY], ey[TY];
+#pragma unroll
+        for (int r = 0; r < TY; ++r) {
+          ex[r] = ey[r] = 0.0;
+          if (do_xy && i < nx && j0 + r < ny) epi_load<MODE>(cb, ebase + (unsigned)r * nx, rsrc, ex[r], ey[r]);
+        }
         double Gyb;
         // y walk: pair terms of ("+") rows (f, f+1) and ("-") rows (f+1, f+2) of gY carried from face to face
         double upb, dp1, Sp1, umb, dm0, Sm0;
@@ -370,49 +447,56 @@ k_flux_vp(const __grid_constant__ CUtensorMap tmap, VPRows<MODEL> rows, ConsRows
           Gyb = Pf + Mf;
         }
         __syncwarp();
-        const size_t ebase = erow + (unsigned)k * pstride + (unsigned)j0 * nx + i;
 #pragma unroll
         for (int r = 0; r < TY; ++r) {
           double acc;
+          const bool st = do_xy && i < nx && j0 + r < ny;
           {
-            // x: left face of cell (lane, r); right face from lane + 1
+            // the six reconstructions of the cell as one batch: x+ x- (left face), y+ y- (face r+1), z+ (face c-1/2), z- (face c-3/2)
             const double* a = pX + r * XW + lane;
             const double* b = mX + r * XW + lane;
-            const double Gl = weno_u(a[0], a[1], a[2]) + weno_u(b[3], b[2], b[1]);
+            const int op = (h * TY + r) * TX, om = ((NHV + h) * TY + r) * TX;
+            const double xa = a[0], xb = a[1], xc = a[2], ya = b[3], yb = b[2], yc = b[1];
+            const double un = pY[(r + 3) * TX], vn = mY[(r + 4) * TX];
+            const double za = zo[op], zb = zm[op], zc = zn[op], wa = zn[om], wb = zm[om], wc = zo[om];
+            const double ul[10] = {xb, xa, yb, ya, upb, umb, zb, za, wb, wa};
+            const double ur[10] = {xc, xb, yc, yb, un, vn, zc, zb, wc, wb};
+            double d[10], S[10];
+            pair_terms_batch<10>(ul, ur, d, S);
+            const double bb[6] = {xb, yb, upb, umb, zb, wb};
+            const double d0[6] = {d[0], d[2], d[4], -dm0, d[6], d[8]};
+            const double d1[6] = {d[1], d[3], dp1, -d[5], d[7], d[9]};
+            const double S0[6] = {S[0], S[2], S[4], Sm0, S[6], S[8]};
+            const double S1[6] = {S[1], S[3], Sp1, S[5], S[7], S[9]};
+            double o[6];
+            weno_ds_batch<6>(bb, d0, d1, S0, S1, o);
+            dp1 = d[4]; Sp1 = S[4]; upb = un;
+            dm0 = d[5]; Sm0 = S[5]; umb = vn;
+            // x: right face from lane + 1
+            const double Gl = o[0] + o[1];
             double Gr = shfl_down1(Gl);
             if (lane == 31) Gr = fX[h * TY + r];
             acc = (Gl - Gr) * hidx;
-            // y: face r + 1 (top of row r)
-            const double un = pY[(r + 3) * TX], vn = mY[(r + 4) * TX];
-            double d0, S0, e1, T1;
-            pair_terms(upb, un, d0, S0);
-            const double Pf = weno_ds(upb, d0, dp1, S0, Sp1);
-            dp1 = d0; Sp1 = S0; upb = un;
-            pair_terms(umb, vn, e1, T1);
-            const double Mf = weno_ds(umb, -dm0, -e1, Sm0, T1);
-            dm0 = e1; Sm0 = T1; umb = vn;
-            const double Gyt = Pf + Mf;
+            // y
+            const double Gyt = o[2] + o[3];
             acc = fma(Gyb - Gyt, hidy, acc);
             Gyb = Gyt;
-          }
-          // z: "+" face c-1/2 stays pending one step, "-" completes face c-3/2
-          {
-            const int op = (h * TY + r) * TX, om = ((NHV + h) * TY + r) * TX;
-            const double Pz = weno_u(zo[op], zm[op], zn[op]);
-            const double Mz = weno_u(zn[om], zm[om], zo[om]);
-            const double G = pend[r] + Mz;
-            pend[r] = Pz;
+            // z: "+" face c-1/2 stays pending one step, "-" completes face c-3/2
+            const double G = pend[r] + o[5];
+            pend[r] = o[4];
             acc = fma(Gprev[r] - G, hidz, acc);
             Gprev[r] = G;
           }
-          if (do_xy && i < nx && j0 + r < ny) store_row<MODE>(L, cb, ebase + (unsigned)r * nx, rsrc, acc);
+          if (st) store_row<MODE>(L, cb, ebase + (unsigned)r * nx, rsrc, acc, ex[r], ey[r]);
         }
       }
+      VP_T(5);
       vp_bar<2, NPA>();                                       // S2: gX, gY and the oldest ring slot are consumed
+      VP_T(6);
     }
   } else {
     // ======================================= Maxwell warps: cell (lane, mw) =======================================
-    const int mw = wrp - WH;
+    const int mw = wrp;
     const int jrow = bc1(j0 + mw, ny, bcy);
     const bool inside = i < nx && j0 + mw < ny;
     // fields of plane c-1 along z, pending "+" faces, previous G (X and Y rows of the 4 pairs)
@@ -424,6 +508,7 @@ k_flux_vp(const __grid_constant__ CUtensorMap tmap, VPRows<MODEL> rows, ConsRows
       const int k = c - 2, t = c - k0;
       const bool staged = t >= 0, do_xy = c >= k0 + 2;
       double* rM = rawM + (t & 1) * GM::RAWM;
+      VP_T(0);
       double zX[4], zY[4];                          // plane c along z: X, Y of the 4 pairs (global memory)
       {
         const unsigned idz = (unsigned)bc1(c, nz, bcz) * pstride + (unsigned)jrow * nx + im;
@@ -437,13 +522,18 @@ k_flux_vp(const __grid_constant__ CUtensorMap tmap, VPRows<MODEL> rows, ConsRows
         if (boundary) mbar_wait_par(&fullH, t & 1);
         mbar_wait_par(&fullM[t & 1], (t >> 1) & 1);
         if (boundary) {
-          vp_fixup<MODEL>(rawH, rM, qin, win, T, bc1(k, nz, bcz), nx, ny, bcx, bcy, NT);
+          vp_fixup<MODEL>(rawH, rM, tab, T, bc1(k, nz, bcz), nx, ny, bcx, bcy, NT);
           vp_bar<0, NT>();
         }
       }
-      double acc[8];
+      VP_T(1);
+      double acc[8], ex[8], ey[8];
+      const size_t e0 = (size_t)((unsigned)k * pstride + (unsigned)(j0 + mw) * nx + i);
 #pragma unroll
-      for (int m = 0; m < 8; ++m) acc[m] = 0.0;
+      for (int m = 0; m < 8; ++m) {
+        acc[m] = 0.0; ex[m] = ey[m] = 0.0;
+        if (do_xy && inside) epi_load<MODE>(cb, (size_t)hm_mrow<MODEL>(m) * N + e0, has_source<MODEL>(hm_mrow<MODEL>(m)), ex[m], ey[m]);
+      }
       const double* cell = rM + (mw + 2) * XW + lane + 2;          // own cell in the staged box
       if (staged) {
         double G33X, G33Y;
@@ -471,55 +561,62 @@ k_flux_vp(const __grid_constant__ CUtensorMap tmap, VPRows<MODEL> rows, ConsRows
               if (y < 4) Pv[y] = s > 0 ? X + Y : X - Y;
               if (y > 0) Mv[y - 1] = s > 0 ? X - Y : X + Y;
             }
-            double dP[3], SP[3], dM[3], SM[3];
-#pragma unroll
-            for (int y = 0; y < 3; ++y) { pair_terms(Pv[y], Pv[y + 1], dP[y], SP[y]); pair_terms(Mv[y], Mv[y + 1], dM[y], SM[y]); }
-            const double Pb = weno_ds(Pv[1], dP[1], dP[0], SP[1], SP[0]), Pt = weno_ds(Pv[2], dP[2], dP[1], SP[2], SP[1]);
-            const double Mb = weno_ds(Mv[1], -dM[0], -dM[1], SM[0], SM[1]), Mt = weno_ds(Mv[2], -dM[1], -dM[2], SM[1], SM[2]);
-            acc[MP::X(n)] = fma((Pb - Mb) - (Pt - Mt), hidy, acc[MP::X(n)]);
-            acc[MP::Y(n)] = fma((Pb + Mb) - (Pt + Mt), s * hidy, acc[MP::Y(n)]);
+            const double ul[6] = {Pv[0], Pv[1], Pv[2], Mv[0], Mv[1], Mv[2]}, ur[6] = {Pv[1], Pv[2], Pv[3], Mv[1], Mv[2], Mv[3]};
+            double d[6], S[6], o[4];
+            pair_terms_batch<6>(ul, ur, d, S);
+            const double bb[4] = {Pv[1], Pv[2], Mv[1], Mv[2]};
+            const double d0[4] = {d[1], d[2], -d[3], -d[4]}, d1[4] = {d[0], d[1], -d[4], -d[5]};
+            const double S0[4] = {S[1], S[2], S[3], S[4]}, S1[4] = {S[0], S[1], S[4], S[5]};
+            weno_ds_batch<4>(bb, d0, d1, S0, S1, o);            // Pb, Pt, Mb, Mt
+            acc[MP::X(n)] = fma((o[0] - o[2]) - (o[1] - o[3]), hidy, acc[MP::X(n)]);
+            acc[MP::Y(n)] = fma((o[0] + o[2]) - (o[1] + o[3]), s * hidy, acc[MP::Y(n)]);
           }
-          {   // x: left face of the cell; right face from lane + 1
-            using MP = MxPair<0>;
-            const double s = MP::s(n);
-            const double* px = cell + MP::X(n) * PL - 2;
-            const double* py = cell + MP::Y(n) * PL - 2;
+          {   // x: left face of the cell (right face from lane + 1);  z: plane c (global), c-1 (registers), c-2 = k (staged box, own cell)
+            using MX = MxPair<0>;
+            using MZ = MxPair<2>;
+            const double sx = MX::s(n), sz = MZ::s(n);
+            const double* px = cell + MX::X(n) * PL - 2;
+            const double* py = cell + MX::Y(n) * PL - 2;
             const double X0 = px[0], X1 = px[1], X2 = px[2], X3 = px[3], Y0 = py[0], Y1 = py[1], Y2 = py[2], Y3 = py[3];
-            const double Po = s > 0 ? weno_u(X0 + Y0, X1 + Y1, X2 + Y2) : weno_u(X0 - Y0, X1 - Y1, X2 - Y2);
-            const double Mo = s > 0 ? weno_u(X3 - Y3, X2 - Y2, X1 - Y1) : weno_u(X3 + Y3, X2 + Y2, X1 + Y1);
-            const double GXl = Po - Mo, GYl = Po + Mo;
+            const double P0 = sx > 0 ? X0 + Y0 : X0 - Y0, P1 = sx > 0 ? X1 + Y1 : X1 - Y1, P2 = sx > 0 ? X2 + Y2 : X2 - Y2;
+            const double M1 = sx > 0 ? X1 - Y1 : X1 + Y1, M2 = sx > 0 ? X2 - Y2 : X2 + Y2, M3 = sx > 0 ? X3 - Y3 : X3 + Y3;
+            const double Xo = cell[MZ::X(n) * PL], Yo = cell[MZ::Y(n) * PL];
+            const double Pn = sz > 0 ? zX[n] + zY[n] : zX[n] - zY[n], Mn = sz > 0 ? zX[n] - zY[n] : zX[n] + zY[n];
+            const double Po_ = sz > 0 ? Xo + Yo : Xo - Yo, Mo_ = sz > 0 ? Xo - Yo : Xo + Yo;
+            const double ul[8] = {P1, P0, M2, M3, mPm[n], Po_, mMm[n], Mn}, ur[8] = {P2, P1, M1, M2, Pn, mPm[n], Mo_, mMm[n]};
+            double d[8], S[8], o[4];
+            pair_terms_batch<8>(ul, ur, d, S);
+            const double bb[4] = {P1, M2, mPm[n], mMm[n]};
+            const double d0[4] = {d[0], d[2], d[4], d[6]}, d1[4] = {d[1], d[3], d[5], d[7]};
+            const double S0[4] = {S[0], S[2], S[4], S[6]}, S1[4] = {S[1], S[3], S[5], S[7]};
+            weno_ds_batch<4>(bb, d0, d1, S0, S1, o);            // x+, x-, z+, z-
+            const double GXl = o[0] - o[1], GYl = o[0] + o[1];
             double GXr = shfl_down1(GXl), GYr = shfl_down1(GYl);
             const double gx33 = shfl_idx(G33X, n), gy33 = shfl_idx(G33Y, n);
             if (lane == 31) { GXr = gx33; GYr = gy33; }
-            acc[MP::X(n)] = fma(GXl - GXr, hidx, acc[MP::X(n)]);
-            acc[MP::Y(n)] = fma(GYl - GYr, s * hidx, acc[MP::Y(n)]);
+            acc[MX::X(n)] = fma(GXl - GXr, hidx, acc[MX::X(n)]);
+            acc[MX::Y(n)] = fma(GYl - GYr, sx * hidx, acc[MX::Y(n)]);
+            const double GX = mpend[n] - o[3], GY = mpend[n] + o[3];
+            mpend[n] = o[2];
+            acc[MZ::X(n)] = fma(mGX[n] - GX, hidz, acc[MZ::X(n)]);
+            acc[MZ::Y(n)] = fma(mGY[n] - GY, sz * hidz, acc[MZ::Y(n)]);
+            mGX[n] = GX; mGY[n] = GY;
+            mPm[n] = Pn; mMm[n] = Mn;
           }
         }
-      }
-      // z: plane c (global), plane c-1 (registers), plane c-2 = k (staged box, own cell)
+      } else {
 #pragma unroll
-      for (int n = 0; n < 4; ++n) {
-        using MP = MxPair<2>;
-        const double s = MP::s(n);
-        const double Pn = s > 0 ? zX[n] + zY[n] : zX[n] - zY[n], Mn = s > 0 ? zX[n] - zY[n] : zX[n] + zY[n];
-        if (staged) {
-          const double Xo = cell[MP::X(n) * PL], Yo = cell[MP::Y(n) * PL];
-          const double Po_ = s > 0 ? Xo + Yo : Xo - Yo, Mo_ = s > 0 ? Xo - Yo : Xo + Yo;
-          const double Pz = weno_u(Po_, mPm[n], Pn);
-          const double Mz = weno_u(Mn, mMm[n], Mo_);
-          const double GX = mpend[n] - Mz, GY = mpend[n] + Mz;
-          mpend[n] = Pz;
-          acc[MP::X(n)] = fma(mGX[n] - GX, hidz, acc[MP::X(n)]);
-          acc[MP::Y(n)] = fma(mGY[n] - GY, s * hidz, acc[MP::Y(n)]);
-          mGX[n] = GX; mGY[n] = GY;
+        for (int n = 0; n < 4; ++n) {   // c = k0 - 1: plane c becomes plane c-1 of the first staged step
+          using MZ = MxPair<2>;
+          const double sz = MZ::s(n);
+          mPm[n] = sz > 0 ? zX[n] + zY[n] : zX[n] - zY[n]; mMm[n] = sz > 0 ? zX[n] - zY[n] : zX[n] + zY[n];
         }
-        mPm[n] = Pn; mMm[n] = Mn;
       }
       if (do_xy && inside) {
-        const size_t e0 = (size_t)((unsigned)k * pstride + (unsigned)(j0 + mw) * nx + i);
 #pragma unroll
-        for (int m = 0; m < 8; ++m) store_row<MODE>(L, cb, (size_t)hm_mrow<MODEL>(m) * N + e0, has_source<MODEL>(hm_mrow<MODEL>(m)), acc[m]);
+        for (int m = 0; m < 8; ++m) store_row<MODE>(L, cb, (size_t)hm_mrow<MODEL>(m) * N + e0, has_source<MODEL>(hm_mrow<MODEL>(m)), acc[m], ex[m], ey[m]);
       }
+      VP_T(5);
       if (staged) mbar_arrive(&doneM[t & 1]);
     }
   }

@@ -845,3 +845,9 @@ int rmhd_probe_hbm(int device, void* stream, long long bytes, double* gbs) {
 }
 
 }  // extern "C"
+
+#ifdef VP_TRACE
+extern "C" int rmhd_debug_trace(long long* out, int n) {
+  return (int)cudaMemcpyFromSymbol(out, rmhd::vp_trace_buf, sizeof(long long) * n);
+}
+#endif
