@@ -1,6 +1,7 @@
 /* =====================================================================================
- * rmhd.h -- C-ABI of librmhd.so: one GPU, FP64, finite-volume IMEX SSP2(222) step for
- * special-relativistic resistive MHD (14 conserved variables) and two-fluid RMHD (18)
+ * rmhd.h -- C-ABI of librmhd.so: one GPU, FP64, finite-volume IMEX step (SSP2(222), Table 2
+ * P:L167-172; SSP3(332), Table 3) for special-relativistic resistive MHD (14
+ * conserved variables) and two-fluid RMHD (18)
  * after Wright & Hawke, "Resistive and multi-fluid RMHD on graphics processing units"
  * (citations "P:Lnnn" are line numbers of the reference text PAPER.md; "Gn" are the
  * readings listed in DESIGN.md).
@@ -64,7 +65,11 @@ typedef struct {
 /* ---- grid simulation (north_star: rmhd_create / set_initial / step / get_state / destroy) -- */
 
 /* Allocate all device state for one grid.  Errors: BAD_PARAM (sizes, ng < 2, mu_e == mu_p,
- * gamma <= 1), CUDA (no device / out of memory). */
+ * gamma <= 1, more than 2^31 - 1 cells), CUDA (no device / out of memory).
+ * One environment switch is read here: RMHD_FLUX=split evaluates L(q) by one pass per axis (the kernels
+ * every 1-D grid uses) instead of the one-pass kernel on 2-D / 3-D grids.  It exists for the parity tests
+ * tests/test_gpu_parity.py::test_ssp3_332_parity[blast_3d_split] and ::test_two_fluid_3d_blast_parity[ssp2-split],
+ * which run those kernels along y and z; it selects no other code. */
 int rmhd_create(const rmhd_params* p, rmhd_ctx** out);
 
 /* Initial primitives -> conserved state (eq 2-4; eq 6), psi = phi = 0
@@ -75,13 +80,16 @@ int rmhd_create(const rmhd_params* p, rmhd_ctx** out);
 int rmhd_set_initial(rmhd_ctx* c, const double* prims, const double* rho_charge, int on_device);
 
 /* Overwrite the conserved state (cons: [14|18][nz][ny][nx]) and recover primitives from it
- * (P:L118-136); prim_guess nullable.  Used for restarts and by tests. */
+ * (P:L118-136); prim_guess ([5|10][nz][ny][nx] hydro primitives) nullable.  Used for restarts and by tests.
+ * Resets the statistics (so the return code, NONCONVERGED if a cell's recovery failed, is this call's
+ * alone); leaves the step counter and rmhd_time untouched. */
 int rmhd_set_cons(rmhd_ctx* c, const double* cons, const double* prim_guess, int on_device);
 
 /* Advance nsteps full IMEX steps (eq 10-11 P:L152-155 read as G1).  SSP2(222), Table 2 P:L167-172:
  * implicit stage, L(q1), implicit stage, L(q2), combine, con2prim.  SSP3(332), Table 3
  * (reading G13): three implicit stages and three L evaluations, same kernels.  Everything runs on
- * the context's stream; one 16-byte device->host read of the failure counters at the end.
+ * the context's stream; one small device->host read of the statistics block (iteration histograms
+ * and failure counters, about 1 KB) and a stream synchronisation at the end.
  * Returns NONCONVERGED if any root-find failed in any cell (the steps are still completed). */
 int rmhd_step(rmhd_ctx* c, int nsteps);
 
@@ -99,7 +107,9 @@ int rmhd_flux_divergence(rmhd_ctx* c, double* Lout, int on_device);
 int rmhd_get_stats(rmhd_ctx* c, long long* hist_stage, long long* hist_c2p, int nbins, long long* n_failed,
                    long long* first_failed_cell);
 
-/* Per-kernel-class device time (CUDA events on the context's stream) accumulated while
+/* Measurement hook (per-kernel fractions beside the whole-step figure; north_star: "evidenced
+ * by ncu counters ... for the implicit and con2prim kernels ... the flux and stage-combine kernels").
+ * Per-kernel-class device time (CUDA events on the context's stream) accumulated while
  * profiling is enabled.  Classes: 0 stage1, 1 stage2, 2 flux sweeps, 3 combine+con2prim,
  * 4 other.  ms[n], launches[n] host arrays. */
 int rmhd_set_profiling(rmhd_ctx* c, int enabled);
@@ -116,6 +126,7 @@ void rmhd_destroy(rmhd_ctx* c);
  * stages them through temporary device buffers (host<->device copies inside the call). */
 
 /* One implicit stage (eq 10):  q* - q_ex - a_dt Psi(q*) = 0 per cell.
+ * (SURVEY.md 8(b) lists `model` and `stream` as arguments: both travel in *p here.)
  * q_ex [14|18][n]; prim_guess [11|16][n] (initial guess: primitives near the solution);
  * sigma_cell [n] per-cell conductivity or NULL (use p->sigma; resistive only);
  * outputs q_out [14|18][n], prims_out [11|16][n], iters [n] Newton iterations taken,
@@ -132,7 +143,8 @@ int rmhd_prim2cons_batch(const rmhd_params* p, long long ncells, const double* p
 int rmhd_con2prim_batch(const rmhd_params* p, long long ncells, const double* cons, const double* prim_guess,
                         double* prims, int* iters, int* fail, int on_device);
 
-/* ---- roofline denominators measured by the library's own probe kernels ------------------- */
+/* ---- roofline denominators measured by the library's own probe kernels (SURVEY.md section 7 step 0:
+ * MEASURED_PEAKS.json holds no FP64 figure, so the FP64 roofline peak is this probe's) ------------- */
 /* FP64 FMA chain on all SMs: returns achieved TFLOP/s (2 flop per DFMA) in *tflops. */
 int rmhd_probe_fp64(int device, void* stream, double* tflops);
 /* Device-to-device streaming copy of `bytes` bytes (read + write counted): GB/s. */

@@ -18,6 +18,7 @@ RMHD_BC_OUTFLOW, RMHD_BC_PERIODIC = 0, 1
 RMHD_OK, RMHD_ERR_BAD_PARAM, RMHD_ERR_CUDA, RMHD_ERR_NONCONVERGED, RMHD_ERR_UNPHYSICAL_INPUT = 0, -1, -2, -3, -4
 NCONS = {0: 14, 1: 18}
 NPRIM = {0: 11, 1: 16}
+NHYD = {0: 5, 1: 10}     # hydro primitive rows (rho, v, p per species); B, E follow
 KERNEL_CLASSES = ("stage1", "stage2", "flux", "combine_c2p", "other")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -138,6 +139,21 @@ def _ptr(x, dtype=np.float64):
     return x.ctypes.data, 0
 
 
+def _numel(x):
+    return int(x.numel()) if _is_torch(x) else int(x.size)
+
+
+def _expect(x, rows, n, what, device=None):
+    """Marshalling check: buffer `x` (None allowed) must hold rows * n elements, and, if it is a CUDA tensor and `device` is given, live
+    on that device.  A wrong size would be an out-of-bounds device access inside the library, not an RMHD_ERR_BAD_PARAM."""
+    if x is None:
+        return
+    if _numel(x) != rows * n:
+        raise ValueError("%s: expected %d x %d elements, got %d" % (what, rows, n, _numel(x)))
+    if device is not None and _is_torch(x) and x.is_cuda and x.device.index != device:
+        raise ValueError("%s lives on cuda:%d, the context on cuda:%d" % (what, x.device.index, device))
+
+
 def _same_side(*flags):
     f = {v for v in flags if v is not None}
     if len(f) > 1:
@@ -217,6 +233,11 @@ def rmhd_time(ctx):
 
 def rmhd_stage_batch(params, q_ex, prim_guess, a_dt, q_out, prims_out, sigma_cell=None, iters=None, fail=None):
     n = q_ex.shape[-1]
+    nc, npr, dev = NCONS[params.model], NPRIM[params.model], params.device
+    _expect(q_ex, nc, n, "q_ex", dev); _expect(q_out, nc, n, "q_out", dev)
+    _expect(prim_guess, npr, n, "prim_guess", dev); _expect(prims_out, npr, n, "prims_out", dev)
+    for x, what in ((sigma_cell, "sigma_cell"), (iters, "iters"), (fail, "fail")):
+        _expect(x, 1, n, what, dev)
     a, d1 = _ptr(q_ex); b, d2 = _ptr(prim_guess); s, d3 = _ptr(sigma_cell)
     qo, d4 = _ptr(q_out); po, d5 = _ptr(prims_out); it, d6 = _ptr(iters, np.int32); fl, d7 = _ptr(fail, np.int32)
     _check(lib().rmhd_stage_batch(C.byref(params), n, a, b, s, float(a_dt), qo, po, it, fl,
@@ -225,12 +246,17 @@ def rmhd_stage_batch(params, q_ex, prim_guess, a_dt, q_out, prims_out, sigma_cel
 
 def rmhd_prim2cons_batch(params, prims, cons, rho_charge=None):
     n = prims.shape[-1]
+    _expect(prims, NPRIM[params.model], n, "prims", params.device); _expect(cons, NCONS[params.model], n, "cons", params.device)
+    _expect(rho_charge, 1, n, "rho_charge", params.device)
     a, d1 = _ptr(prims); r, d2 = _ptr(rho_charge); c, d3 = _ptr(cons)
     _check(lib().rmhd_prim2cons_batch(C.byref(params), n, a, r, c, _same_side(d1, d2, d3)))
 
 
 def rmhd_con2prim_batch(params, cons, prims, prim_guess=None, iters=None, fail=None):
     n = cons.shape[-1]
+    _expect(cons, NCONS[params.model], n, "cons", params.device); _expect(prims, NPRIM[params.model], n, "prims", params.device)
+    _expect(prim_guess, NPRIM[params.model], n, "prim_guess", params.device)
+    _expect(iters, 1, n, "iters", params.device); _expect(fail, 1, n, "fail", params.device)
     a, d1 = _ptr(cons); g, d2 = _ptr(prim_guess); w, d3 = _ptr(prims)
     it, d4 = _ptr(iters, np.int32); fl, d5 = _ptr(fail, np.int32)
     _check(lib().rmhd_con2prim_batch(C.byref(params), n, a, g, w, it, fl, _same_side(d1, d2, d3, d4, d5)))
@@ -272,10 +298,19 @@ class Rmhd:
     dt = property(lambda self: rmhd_dt(self.ctx))
     time = property(lambda self: rmhd_time(self.ctx))
 
+    @property
+    def ncells(self):
+        return self.shape[0] * self.shape[1] * self.shape[2]
+
     def set_initial(self, prims, rho_charge=None):
+        _expect(prims, NPRIM[self.model], self.ncells, "prims", self.params.device)
+        _expect(rho_charge, 1, self.ncells, "rho_charge", self.params.device)
         rmhd_set_initial(self.ctx, prims, rho_charge)
 
     def set_cons(self, cons, prim_guess=None):
+        _expect(cons, NCONS[self.model], self.ncells, "cons", self.params.device)
+        if prim_guess is not None and _numel(prim_guess) not in (NHYD[self.model] * self.ncells, NPRIM[self.model] * self.ncells):
+            raise ValueError("prim_guess: expected the %d hydro rows (or all %d primitive rows) per cell" % (NHYD[self.model], NPRIM[self.model]))
         return rmhd_set_cons(self.ctx, cons, prim_guess)
 
     def step(self, n=1, check=True):

@@ -13,7 +13,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librmhd.so")
 SOURCES = [os.path.join(CSRC, "rmhd.cu")]
-HEADERS = [os.path.join(CSRC, f) for f in ("physics.cuh", "stage.cuh", "kernels.cuh", "flux_fused.cuh", "flux_hm.cuh", "flux_vp.cuh")] + [os.path.join(ROOT, "include", "rmhd.h")]
+HEADERS = [os.path.join(CSRC, f) for f in ("physics.cuh", "stage.cuh", "kernels.cuh", "flux_fused.cuh", "flux_hm.cuh")] + [os.path.join(ROOT, "include", "rmhd.h")]
 
 
 def _stale():

@@ -222,7 +222,6 @@ __global__ void __launch_bounds__(128, 5) k_stage_resistive(const double* __rest
         qe[v] = fma(k.cP[0], Ps1[(size_t)j * N + c], qe[v]);
         if (NL >= 2 && k.cP[1] != 0.0) qe[v] = fma(k.cP[1], Ps2[(size_t)j * N + c], qe[v]);
       }
-#pragma unroll
       if (!(NL == 1 && k.pre)) {
 #pragma unroll
         for (int v = 0; v < R_NC; ++v) if (v < 8 || v == 11) qs[(size_t)v * N + c] = qe[v];
@@ -342,7 +341,6 @@ __global__ void __launch_bounds__(128) k_stage_two_fluid(const double* __restric
         qe[v] = fma(k.cP[0], Ps1[(size_t)j * N + c], qe[v]);
         if (NL >= 2 && k.cP[1] != 0.0) qe[v] = fma(k.cP[1], Ps2[(size_t)j * N + c], qe[v]);
       }
-#pragma unroll
       if (!(NL == 1 && k.pre)) {
 #pragma unroll
         for (int v = 0; v < T_NC; ++v) if (v < 6 || (v >= 10 && v < 13)) qs[(size_t)v * N + c] = qe[v];

@@ -11,7 +11,6 @@
 #include "kernels.cuh"
 #include "flux_fused.cuh"
 #include "flux_hm.cuh"
-#include "flux_vp.cuh"
 
 using namespace rmhd;
 
@@ -39,16 +38,9 @@ struct rmhd_ctx {
   Stats* d_stats;
   Stats* h_stats;  // pinned
   bool profiling;
-  bool fused_flux;   // one-pass L(q) over all axes (flux_fused.cuh) when nx, ny > 1; RMHD_FLUX=split forces the per-axis kernels
-  bool fuse_combine; // eq (11) in the epilogue of the F2 flux launch (fused path only); RMHD_COMBINE=split keeps k_final
-  int hm_ty;         // tile rows of the two-role flux kernel: 8 (one 16-warp CTA per SM; default when ny >= 8) or 4 (two CTAs); RMHD_HM_TY
-  bool march2d;      // resistive 2-D grids through the marching two-role kernel (default); RMHD_FLUX2D=tile keeps one plane per CTA
-  bool comb_mix;     // rows without a source: A rebuilt in the flux epilogue from qn and the last stage state; RMHD_COMBINE=full stores all of A
-  bool pre_s2;       // SSP2 fused path: F1 stores q_ex of stage 2 for the rows without a source; RMHD_PRE=0 disables
-  bool one_role;     // RMHD_FLUX=fused1: resistive model through the one-thread-per-column kernel (flux_fused.cuh) instead of flux_hm.cuh
+  bool fused_flux;   // one-pass L(q) over all axes (flux_hm.cuh) when nx, ny > 1; RMHD_FLUX=split (see rmhd.h) forces the per-axis kernels
+  int hm_ty;         // tile rows of the two-role flux kernel: 8 (one 16-warp CTA per SM) when ny >= 8, else 4 (two CTAs)
   int sm_count;
-  bool vp_ok;        // 3-D resistive grids with even nx: the TMA-staged, variable-specialised flux kernel (flux_vp.cuh)
-  CUtensorMap tmap;  // 4-D view (x, y, z, row) of the whole state allocation, box = one haloed tile plane of one row
   std::vector<EvRec> pending;
   std::vector<cudaEvent_t> ev_pool;
   double ms[KC_N];
@@ -121,16 +113,12 @@ void resolve_events(rmhd_ctx* c) {  // stream must be synchronised
 // ---- launches ----------------------------------------------------------------------------
 template <int MODEL, int AXIS>
 int launch_flux_axis(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODEL>& wr, double* L, int accumulate) {
-  static bool attr_set[8] = {false, false, false, false, false, false, false, false};
   const int nx = c->n[0], ny = c->n[1], nz = c->n[2];
   const int ns = c->n[AXIS];
   if constexpr (AXIS == 0) {
     constexpr int TS = Tile<AXIS>::TS, TO = Tile<AXIS>::TO;
     const size_t smem = flux_smem_bytes<MODEL, AXIS>();
-    if (!attr_set[c->device & 7]) {
-      CK(c, cudaFuncSetAttribute(k_flux<MODEL, AXIS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      attr_set[c->device & 7] = true;
-    }
+    CK(c, cudaFuncSetAttribute(k_flux<MODEL, AXIS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dim3 grid((ny * nz + TO - 1) / TO, (ns + TS - 1) / TS, 1);
     if (ny * nz == 1) grid = dim3(1, (ns + TS * TO - 1) / (TS * TO), 1);   // 1-D: the tile rows are laid along x
     Timed t(c, KC_FLUX);
@@ -138,10 +126,7 @@ int launch_flux_axis(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODEL
     CK(c, cudaGetLastError());
   } else {
     const size_t smem = march_smem_bytes<MODEL>();
-    if (!attr_set[c->device & 7]) {
-      CK(c, cudaFuncSetAttribute(k_flux_march<MODEL, AXIS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-      attr_set[c->device & 7] = true;
-    }
+    CK(c, cudaFuncSetAttribute(k_flux_march<MODEL, AXIS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     // segments along the sweep axis: enough threads for ~8 resident waves-worth of columns, segments >= 8 cells
     const long long columns = (long long)((nx + MARCH_THREADS - 1) / MARCH_THREADS) * MARCH_THREADS * (AXIS == 1 ? nz : ny);
     const long long want_threads = 148LL * 384 * 4;
@@ -159,25 +144,18 @@ int launch_flux_axis(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODEL
   return RMHD_OK;
 }
 
-// all present axes in one pass (flux_fused.cuh, flux_hm.cuh); needs nx > 1 and ny > 1.  TYP: tile rows of the two-role kernel
+// all present axes in one pass (flux_hm.cuh); needs nx > 1 and ny > 1.  TYP: tile rows of the two-role kernel
 template <int MODEL, bool HAS_Z, bool COMB, int TYP>
 int launch_flux_fused(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODEL>& wr, double* L, const FluxComb& cb) {
-  static bool attr_set[8] = {false, false, false, false, false, false, false, false};
   const int nx = c->n[0], ny = c->n[1], nz = c->n[2];
-  const bool two_role = !c->one_role;
-  const int ty = two_role ? TYP : FF_TY;
-  const size_t smem = two_role ? HMGeom<TYP, MODEL>::bytes(HAS_Z) : FFSmem<MODEL>::bytes(HAS_Z);
-  if (!attr_set[c->device & 7]) {
-    CK(c, cudaFuncSetAttribute(k_flux_fused<MODEL, HAS_Z, COMB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FFSmem<MODEL>::bytes(HAS_Z)));
-    CK(c, cudaFuncSetAttribute(k_flux_hm<HAS_Z, COMB, TYP, true, 2, MODEL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)HMGeom<TYP, MODEL>::bytes(HAS_Z)));
-    attr_set[c->device & 7] = true;
-  }
-  const int gx = (nx + FF_TX - 1) / FF_TX, gy = (ny + ty - 1) / ty;
+  const size_t smem = HMGeom<TYP, MODEL>::bytes(HAS_Z);
+  CK(c, cudaFuncSetAttribute(k_flux_hm<HAS_Z, COMB, TYP, true, 2, MODEL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const int gx = (nx + FF_TX - 1) / FF_TX, gy = (ny + TYP - 1) / TYP;
   int nseg = 1, seg_len = 1;
   if (HAS_Z) {
     // z segments: pick the count (segments of >= 16 planes) that wastes least, counting the partially filled
     // last wave of resident CTAs and the 4 feed-only prologue planes of every segment
-    const bool one_cta = two_role && (TYP == 8 || MODEL == 1);
+    const bool one_cta = TYP == 8 || MODEL == 1;
     const long long tiles = (long long)gx * gy, slots = (one_cta ? 1LL : 2LL) * c->sm_count;
     double best = 1e300;
     for (int s = 1; s <= (nz + 15) / 16 && s <= 64; ++s) {
@@ -189,12 +167,8 @@ int launch_flux_fused(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODE
   }
   dim3 grid(gx, gy, nseg);
   Timed t(c, KC_FLUX);
-  if (two_role)
-    k_flux_hm<HAS_Z, COMB, TYP, true, 2, MODEL><<<grid, HMGeom<TYP, MODEL>::THREADS, smem, c->stream>>>(
-        qr, wr, L, c->N, nx, ny, nz, c->p.bc[0], c->p.bc[1], c->p.bc[2], 0.5 / c->dx[0], 0.5 / c->dx[1], 0.5 / c->dx[2], seg_len, c->P, cb);
-  else
-    k_flux_fused<MODEL, HAS_Z, COMB><<<grid, FF_THREADS, smem, c->stream>>>(qr, wr, L, c->N, nx, ny, nz, c->p.bc[0], c->p.bc[1], c->p.bc[2],
-                                                                           0.5 / c->dx[0], 0.5 / c->dx[1], 0.5 / c->dx[2], seg_len, c->P, cb);
+  k_flux_hm<HAS_Z, COMB, TYP, true, 2, MODEL><<<grid, HMGeom<TYP, MODEL>::THREADS, smem, c->stream>>>(
+      qr, wr, L, c->N, nx, ny, nz, c->p.bc[0], c->p.bc[1], c->p.bc[2], 0.5 / c->dx[0], 0.5 / c->dx[1], 0.5 / c->dx[2], seg_len, c->P, cb);
   CK(c, cudaGetLastError());
   return RMHD_OK;
 }
@@ -210,14 +184,10 @@ int launch_flux_fused(rmhd_ctx* c, const ConsRows<MODEL>& qr, const HydRows<MODE
 // (flux_hm.cuh, HAS_Y = false, ZDIR = 1)
 template <bool COMB>
 int launch_flux_march2d(rmhd_ctx* c, const ConsRows<0>& qr, const HydRows<0>& wr, double* L, const FluxComb& cb) {
-  static bool attr_set[8] = {false, false, false, false, false, false, false, false};
   constexpr int TYP = 8;
   const int nx = c->n[0], ny = c->n[1];
   const size_t smem = HMGeom<TYP>::bytes(true);
-  if (!attr_set[c->device & 7]) {
-    CK(c, cudaFuncSetAttribute(k_flux_hm<true, COMB, TYP, false, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_set[c->device & 7] = true;
-  }
+  CK(c, cudaFuncSetAttribute(k_flux_hm<true, COMB, TYP, false, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const int gx = (nx + FF_TX * TYP - 1) / (FF_TX * TYP);
   // segments along y: fill the SMs (one CTA each), at least 4 planes per segment, then the same waste measure as in 3-D
   int nseg = 1, seg_len = ny;
@@ -239,62 +209,6 @@ int launch_flux_march2d(rmhd_ctx* c, const ConsRows<0>& qr, const HydRows<0>& wr
   return RMHD_OK;
 }
 
-// 3-D grids, resistive model: TMA-staged planes, one warp per row with a non-trivial flux (flux_vp.cuh)
-template <int MODE>
-int launch_flux_vp(rmhd_ctx* c, const ConsRows<0>& qr, const HydRows<0>& wr, double* L, const FluxComb& cb) {
-  using GM = VPGeom<0>;
-  using FS = FSet<0>;
-  static bool attr_set[8] = {false, false, false, false, false, false, false, false};
-  const int nx = c->n[0], ny = c->n[1], nz = c->n[2];
-  const size_t smem = GM::bytes();
-  if (!attr_set[c->device & 7]) {
-    CK(c, cudaFuncSetAttribute(k_flux_vp<MODE, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    attr_set[c->device & 7] = true;
-  }
-  VPRows<0> rows;
-  auto row_of = [&](const double* p) { return (int)((size_t)(p - c->q) / c->N); };
-  for (int h = 0; h < GM::NHV; ++h) rows.h[h] = row_of(qr.r[FS::hv(h)]);
-  for (int v = 0; v < GM::NH; ++v) rows.h[GM::NHV + v] = row_of(wr.r[v]);
-  for (int m = 0; m < 8; ++m) rows.m[m] = row_of(qr.r[hm_mrow<0>(m)]);
-  const int gx = (nx + VP_TX - 1) / VP_TX, gy = (ny + VP_TY - 1) / VP_TY;
-  // z segments: the count (segments of >= 16 planes) that wastes least, counting the partially filled last wave of CTAs
-  // (one per SM) and the 4 feed-only planes of every segment
-  int nseg = 1, seg_len = nz;
-  {
-    const long long tiles = (long long)gx * gy, slots = c->sm_count;
-    double best = 1e300;
-    for (int s = 1; s <= (nz + 15) / 16 && s <= 64; ++s) {
-      const int len = (nz + s - 1) / s, cnt = (nz + len - 1) / len;
-      const long long ctas = tiles * cnt, waves = (ctas + slots - 1) / slots;
-      const double cost = (double)waves * slots / (double)ctas * (1.0 + 3.0 / len);
-      if (cost < best - 1e-9) { best = cost; nseg = cnt; seg_len = len; }
-    }
-  }
-  dim3 grid(gx, gy, nseg);
-  Timed t(c, KC_FLUX);
-  k_flux_vp<MODE, 0><<<grid, GM::THREADS, smem, c->stream>>>(c->tmap, rows, qr, wr, L, c->N, nx, ny, nz, c->p.bc[0], c->p.bc[1], c->p.bc[2],
-                                                            0.5 / c->dx[0], 0.5 / c->dx[1], 0.5 / c->dx[2], seg_len, c->P, cb);
-  CK(c, cudaGetLastError());
-  return RMHD_OK;
-}
-
-// tensor map of the state allocation for flux_vp.cuh (driver entry point through the runtime: no -lcuda)
-int make_tensor_map(rmhd_ctx* c, size_t rows) {
-  typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
-                               const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-  void* fn = nullptr;
-  cudaDriverEntryPointQueryResult qres;
-  CK(c, cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
-  if (!fn || qres != cudaDriverEntryPointSuccess) { c->err = "cuTensorMapEncodeTiled not available"; return RMHD_ERR_CUDA; }
-  const cuuint64_t dims[4] = {(cuuint64_t)c->n[0], (cuuint64_t)c->n[1], (cuuint64_t)c->n[2], (cuuint64_t)rows};
-  const cuuint64_t strides[3] = {sizeof(double) * (cuuint64_t)c->n[0], sizeof(double) * (cuuint64_t)c->n[0] * c->n[1], sizeof(double) * (cuuint64_t)c->N};
-  const cuuint32_t box[4] = {VP_XW, VP_YR, 1, 1}, est[4] = {1, 1, 1, 1};
-  const CUresult r = ((EncodeFn)fn)(&c->tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, c->q, dims, strides, box, est, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                                    CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-  if (r != CUDA_SUCCESS) { char b[96]; snprintf(b, sizeof b, "cuTensorMapEncodeTiled failed (%d)", (int)r); c->err = b; return RMHD_ERR_CUDA; }
-  return RMHD_OK;
-}
-
 inline bool uses_fused_flux(const rmhd_ctx* c) { return c->fused_flux && c->n[0] > 1 && c->n[1] > 1; }
 
 // `cb` (fused path only): store the eq-(11) update of q instead of L (a5 fused into F2)
@@ -308,12 +222,7 @@ int launch_flux(rmhd_ctx* c, const double* qa, const double* qb, bool mix, const
   if (uses_fused_flux(c)) {
     const FluxComb none = {nullptr, nullptr, 0.0, nullptr, 0.0, 0};
     if constexpr (MODEL == 0) {
-      if (c->vp_ok) {
-        if (!cb) return launch_flux_vp<0>(c, qr, wr, L, none);
-        if (cb->pre) return launch_flux_vp<1>(c, qr, wr, L, *cb);
-        if (cb->theta > 0.0) return launch_flux_vp<2>(c, qr, wr, L, *cb);
-      }
-      if (c->n[2] == 1 && c->march2d && !c->one_role) return cb ? launch_flux_march2d<true>(c, qr, wr, L, *cb) : launch_flux_march2d<false>(c, qr, wr, L, none);
+      if (c->n[2] == 1) return cb ? launch_flux_march2d<true>(c, qr, wr, L, *cb) : launch_flux_march2d<false>(c, qr, wr, L, none);
     }
     if (cb) return c->n[2] > 1 ? launch_flux_fused<MODEL, true, true>(c, qr, wr, L, *cb) : launch_flux_fused<MODEL, false, true>(c, qr, wr, L, *cb);
     return c->n[2] > 1 ? launch_flux_fused<MODEL, true, false>(c, qr, wr, L, none) : launch_flux_fused<MODEL, false, false>(c, qr, wr, L, none);
@@ -354,9 +263,9 @@ int step_once(rmhd_ctx* c) {
   StageCoef k1 = {};
   k1.a = g * dt;
   if ((rc = launch_stage<MODEL, 0, false>(c, KC_STAGE1, k1, c->Ps1, nullptr))) return rc;
-  const bool fuse_c = uses_fused_flux(c) && c->fuse_combine;
+  const bool fuse_c = uses_fused_flux(c);
   // F1 on the fused path also leaves q_ex of stage 2 for the rows without a source (qn + dt L1) in the stage-state buffer
-  const bool pre = fuse_c && c->comb_mix && c->pre_s2;
+  const bool pre = fuse_c;
   if (pre) {
     const FluxComb cb1 = {c->qs, nullptr, dt, c->q, 0.0, 1};
     if ((rc = launch_flux<MODEL>(c, c->q, c->qs, true, c->w, c->L1, &cb1))) return rc;
@@ -368,9 +277,9 @@ int step_once(rmhd_ctx* c) {
   if (fuse_c) {
     // stage 2 leaves A = qn + dt/2 L1 + dt/2 (Psi1 + Psi2) in the L2 buffer; F2 + C in one launch
     // (q^{n+1} = A + dt/2 L2 row by row in the flux kernel's epilogue), then P
-    k2.a_src_only = c->comb_mix;
+    k2.a_src_only = true;
     if ((rc = launch_stage<MODEL, 1, true>(c, KC_STAGE2, k2, nullptr, c->L2))) return rc;
-    const FluxComb cb = {c->q, c->L2, 0.5 * dt, c->qs, c->comb_mix ? 0.5 : 0.0, 0};
+    const FluxComb cb = {c->q, c->L2, 0.5 * dt, c->qs, 0.5, 0};
     if ((rc = launch_flux<MODEL>(c, c->qs, nullptr, false, c->w, c->L2, &cb))) return rc;
     return launch_con2prim<MODEL>(c);
   }
@@ -404,12 +313,12 @@ int step_once_ssp3(rmhd_ctx* c) {
   StageCoef k3 = {};
   k3.a = g * dt; k3.cL[0] = 0.25 * dt; k3.cL[1] = 0.25 * dt; k3.cP[0] = (0.5 - g) * dt; k3.cP[1] = 0.0;
   k3.hL[0] = dt / 6.0; k3.hL[1] = dt / 6.0; k3.hP[0] = dt / 6.0; k3.hP[1] = dt / 6.0; k3.hP[2] = 2.0 * dt / 3.0;
-  const bool fuse3 = uses_fused_flux(c) && c->fuse_combine;
-  k3.a_src_only = fuse3 && c->comb_mix;
+  const bool fuse3 = uses_fused_flux(c);
+  k3.a_src_only = fuse3;
   if ((rc = launch_stage<MODEL, 2, true>(c, KC_STAGE2, k3, nullptr, c->A))) return rc;
   const double wl = 2.0 * dt / 3.0;
   if (fuse3) {
-    const FluxComb cb = {c->q, c->A, wl, c->qs, c->comb_mix ? 2.0 / 3.0 : 0.0, 0};
+    const FluxComb cb = {c->q, c->A, wl, c->qs, 2.0 / 3.0, 0};
     if ((rc = launch_flux<MODEL>(c, c->qs, nullptr, false, c->w, c->L1, &cb))) return rc;
     return launch_con2prim<MODEL>(c);
   }
@@ -475,13 +384,8 @@ int rmhd_create(const rmhd_params* p, rmhd_ctx** out) {
   c->dt = inv > 0.0 ? p->cfl / inv : p->cfl;   // G9
   c->nsteps = 0; c->device = p->device; c->stream = (cudaStream_t)p->stream;
   c->profiling = false;
-  { const char* e = getenv("RMHD_FLUX"); c->fused_flux = !(e && strcmp(e, "split") == 0); }
-  { const char* e = getenv("RMHD_FLUX"); c->one_role = e && strcmp(e, "fused1") == 0; }
-  { const char* e = getenv("RMHD_COMBINE"); c->fuse_combine = !(e && strcmp(e, "split") == 0); }
-  { const char* e = getenv("RMHD_COMBINE"); c->comb_mix = !(e && strcmp(e, "full") == 0); }
-  { const char* e = getenv("RMHD_PRE"); c->pre_s2 = !(e && strcmp(e, "0") == 0); }
-  { const char* e = getenv("RMHD_FLUX2D"); c->march2d = !(e && strcmp(e, "tile") == 0); }
-  { const char* e = getenv("RMHD_HM_TY"); c->hm_ty = e ? (atoi(e) == 8 ? 8 : 4) : (p->ny >= 8 ? 8 : 4); }
+  { const char* e = getenv("RMHD_FLUX"); c->fused_flux = !(e && strcmp(e, "split") == 0); }   // documented in rmhd.h
+  c->hm_ty = p->ny >= 8 ? 8 : 4;
   c->sm_count = 148;
   for (int i = 0; i < KC_N; ++i) { c->ms[i] = 0.0; c->launches[i] = 0; }
   c->q = c->w = c->qs = c->L1 = c->L2 = c->Ps1 = c->Ps2 = c->A = nullptr; c->d_stats = nullptr; c->h_stats = nullptr;
@@ -500,15 +404,6 @@ int rmhd_create(const rmhd_params* p, rmhd_ctx** out) {
   b += (size_t)c->nh * c->N; c->Ps1 = b;
   b += (size_t)c->ns * c->N; c->Ps2 = b;
   if (p->integrator == RMHD_SSP3_332) { b += (size_t)c->ns * c->N; c->A = b; }
-  c->vp_ok = false;
-  {
-    const char* ev = getenv("RMHD_FLUX");
-    const bool want = !(ev && (strcmp(ev, "hm") == 0 || strcmp(ev, "split") == 0 || strcmp(ev, "fused1") == 0));
-    if (want && p->model == RMHD_RESISTIVE && p->nx > 1 && p->ny > 1 && p->nz > 1 && p->nx % 2 == 0) {
-      if (make_tensor_map(c, rows)) { g_create_error = c->err; rmhd_destroy(c); return RMHD_ERR_CUDA; }
-      c->vp_ok = true;
-    }
-  }
   e = cudaMemsetAsync(c->q, 0, sizeof(double) * rows * c->N, c->stream);
   if (e != cudaSuccess) { fail_cuda(nullptr, e, "clearing device state"); rmhd_destroy(c); return RMHD_ERR_CUDA; }
   if (reset_stats(c)) { g_create_error = c->err; rmhd_destroy(c); return RMHD_ERR_CUDA; }
@@ -567,6 +462,7 @@ int rmhd_set_cons(rmhd_ctx* c, const double* cons, const double* prim_guess, int
   DeviceGuard dg(c->device);
   const size_t N = c->N;
   CK(c, cudaMemcpyAsync(c->q, cons, sizeof(double) * c->nc * N, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
+  { int rc0 = reset_stats(c); if (rc0) return rc0; }
   const double* d_guess = prim_guess;
   if (prim_guess && !on_device) {
     CK(c, cudaMemcpyAsync(c->qs, prim_guess, sizeof(double) * c->nh * N, cudaMemcpyHostToDevice, c->stream));
@@ -845,9 +741,3 @@ int rmhd_probe_hbm(int device, void* stream, long long bytes, double* gbs) {
 }
 
 }  // extern "C"
-
-#ifdef VP_TRACE
-extern "C" int rmhd_debug_trace(long long* out, int n) {
-  return (int)cudaMemcpyFromSymbol(out, rmhd::vp_trace_buf, sizeof(long long) * n);
-}
-#endif

@@ -420,9 +420,9 @@ def test_paper_setups_parity(B, O, synth, case, integrator):
     assert rel_l1(w[:nh], wo[:nh]) <= 10 * tol
 
 
-@pytest.mark.parametrize("integrator,flux", [("ssp2", None), ("ssp3", None), ("ssp2", "fused1"), ("ssp2", "split")])
+@pytest.mark.parametrize("integrator,flux", [("ssp2", None), ("ssp3", None), ("ssp2", "split")])
 def test_two_fluid_3d_blast_parity(B, O, synth, integrator, flux, monkeypatch):
-    """Full steps of the 18-variable model in 3-D (two-role flux kernel, one-role kernel, per-axis kernels)."""
+    """Full steps of the 18-variable model in 3-D (two-role flux kernel, per-axis kernels)."""
     if flux:
         monkeypatch.setenv("RMHD_FLUX", flux)
     c = synth.two_fluid_blast(n=36, nsteps=8, integrator=integrator)
