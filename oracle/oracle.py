@@ -73,6 +73,7 @@ def lib():
         L.oracle_eval_L.argtypes = [C.c_void_p, _dp]
         L.oracle_get_stats.argtypes = [C.c_void_p, _lp, _lp, C.c_int, _lp, _lp]
         L.oracle_set_threads.argtypes = [C.c_int]
+        L.oracle_set_c2p_switch.argtypes = [C.c_int]
         L.oracle_prim2cons_batch.argtypes = [C.POINTER(OracleParams), C.c_longlong, _dp, _dp, _dp]
         L.oracle_con2prim_batch.argtypes = [C.POINTER(OracleParams), C.c_longlong, _dp, _dp, _dp, _ip, _ip]
         L.oracle_flux_vector_batch.argtypes = [C.POINTER(OracleParams), C.c_longlong, C.c_int, _dp, _dp, _dp, _dp]
@@ -99,6 +100,11 @@ def _c(a):
 def set_threads(n=0):
     """n > 0 sets the OpenMP thread count; returns the count in force."""
     return lib().oracle_set_threads(int(n))
+
+
+def set_c2p_switch(n=20):
+    """Iterations of the first con2prim residual before the second (quartic in W) takes over; 0 = second only.  Returns the previous value."""
+    return lib().oracle_set_c2p_switch(int(n))
 
 
 # ---- batched per-cell operations -------------------------------------------------------

@@ -93,6 +93,58 @@ struct Hydro {
 // for Gamma <= 2).  Stop when the applied update |dZ| <= tol * Z (G5: the paper's 1e-13
 // read as a relative step tolerance; the update is applied, so the root sits at round-off).
 // returns 0 ok, 1 inadmissible input, 2 not converged, 3 unphysical result
+// Second residual (two alternative residuals, "one may converge where the other may not"; the paper cites
+// them without printing them, G4).  Reading taken: the same recovery written in the Lorentz factor W instead of Z, which
+// for the Gamma-law EOS (eq 4) is a quartic.  With E := taut + D = Z - p and p = g (Z / W^2 - D / W), g = (G-1)/G:
+//   Z(W) = W (E W - g D) / (W^2 - g),
+// and St^2 = Z^2 (1 - 1/W^2) gives
+//   F(W) = (E W - g D)^2 (W^2 - 1) - St^2 (W^2 - g)^2 = 0   on  1 <= W <= Wmax = (1 - St^2/E^2)^(-1/2)  (p >= 0 <=> Z >= E).
+// F(1) = -St^2 (1 - g)^2 <= 0; an admissible state has F(Wmax) >= 0.  Newton-Raphson from W = Wmax kept inside the
+// bracket (bisection otherwise); stop when the applied update |dW| <= tol W, or when |F| has reached its round-off floor
+// 32 eps ((E W - g D)^2 (W^2 - 1) + St^2 (W^2 - g)^2) (the two terms cancel to ~(E - |St|)/E where this residual is
+// needed, so the update cannot shrink further).  It is the automatic fall-back of c2p_hydro
+// below after g_c2p_switch iterations of the first residual: near |St| -> E (large W, hot gas) f(Z) is almost flat at the
+// root while F(W) stays a well-scaled polynomial.
+int g_c2p_switch = 20;   // iterations of the first residual before the second takes over (0: second residual only; test hook)
+
+int c2p_hydro_W(double D, const double* St, double taut, double gam, double tol, int maxit, Hydro& w, int& iters) {
+  const double g = (gam - 1.0) / gam;
+  const double S2 = dot3(St, St);
+  const double Sabs = std::sqrt(S2);
+  const double E = taut + D;
+  auto F = [&](double W, double& dF, double& mag) {
+    const double a = E * W - g * D, b = W * W - g, c = W * W - 1.0;
+    dF = 2.0 * E * a * c + 2.0 * W * a * a - 4.0 * S2 * W * b;
+    mag = a * a * c + S2 * b * b;
+    return a * a * c - S2 * b * b;
+  };
+  const double floor_eps = 32.0 * std::numeric_limits<double>::epsilon();
+  double lo = 1.0, hi = 1.0 / std::sqrt((E - Sabs) * (E + Sabs) / (E * E));
+  double dF, mag;
+  if (!std::isfinite(hi) || !(F(hi, dF, mag) >= -floor_eps * mag)) return 3;          // no root with p >= 0
+  double W = hi;
+  bool conv = false;
+  while (iters < maxit) {
+    ++iters;
+    const double f = F(W, dF, mag);
+    if (std::fabs(f) <= floor_eps * mag) { conv = true; break; }
+    if (f < 0.0) lo = std::max(lo, W); else hi = std::min(hi, W);
+    double Wn = W - f / dF;
+    if (!(Wn >= lo && Wn <= hi) || !std::isfinite(Wn)) Wn = 0.5 * (lo + hi);
+    const double dW = Wn - W;
+    W = Wn;
+    if (std::fabs(dW) <= tol * W) { conv = true; break; }
+  }
+  const double Z = W * (E * W - g * D) / (W * W - g);
+  w.Z = Z; w.W = W;
+  w.p = g * (Z / (W * W) - D / W);
+  w.rho = D / W;
+  for (int i = 0; i < 3; ++i) w.v[i] = St[i] / Z;
+  if (!conv) return 2;
+  if (!(w.p > 0.0) || !(w.rho > 0.0) || !std::isfinite(w.p) || !std::isfinite(Z)) return 3;
+  return 0;
+}
+
 int c2p_hydro(double D, const double* St, double taut, double gam, double Zguess, double tol, int maxit,
               Hydro& w, int& iters) {
   const double g = (gam - 1.0) / gam;
@@ -107,6 +159,7 @@ int c2p_hydro(double D, const double* St, double taut, double gam, double Zguess
   if (!(Z > Sabs) || !std::isfinite(Z)) Z = std::max(taut + D, Sabs * (1.0 + 1e-8) + 1e-300);
   bool conv = false;
   for (int it = 1; it <= maxit; ++it) {
+    if (it > g_c2p_switch) return c2p_hydro_W(D, St, taut, gam, tol, maxit, w, iters);
     iters = it;
     double v2 = S2 / (Z * Z);
     double om = 1.0 - v2;
@@ -959,6 +1012,9 @@ void* oracle_create(const oracle_params* p) {
   S->n_failed = 0; S->first_failed = -1;
   return S;
 }
+
+// test hook: iterations of the first con2prim residual before the second takes over (default 20; 0 = second only)
+int oracle_set_c2p_switch(int n) { int prev = g_c2p_switch; g_c2p_switch = n; return prev; }
 
 void oracle_destroy(void* h) { delete static_cast<Sim*>(h); }
 double oracle_dt(void* h) { return static_cast<Sim*>(h)->dt; }

@@ -240,3 +240,21 @@ def random_two_fluid_prims(n, seed, vmax=0.9):
     B = rng.standard_normal((3, n))
     E = rng.standard_normal((3, n))
     return np.ascontiguousarray(np.concatenate(parts + [B, E], axis=0))
+
+
+def stress_resistive_prims(n, seed, w_max=100.0, noise=1e-3):
+    """Hard tail for con2prim: Lorentz factors log-uniform up to `w_max`, p/rho log-uniform
+    in [1e-8, 1e4], B^2/rho log-uniform in [1e-4, 1e4], E = -v x B (1 + noise N(0,1)) component-wise, rho log-uniform in
+    [1e-3, 1e3].  Initial data only: no method arithmetic."""
+    rng = np.random.default_rng(seed)
+    rho = 10.0 ** rng.uniform(-3.0, 3.0, n)
+    p = rho * 10.0 ** rng.uniform(-8.0, 4.0, n)
+    W = 10.0 ** rng.uniform(0.0, np.log10(w_max), n)
+    dirs = rng.standard_normal((3, n))
+    dirs /= np.sqrt((dirs ** 2).sum(axis=0))
+    v = dirs * np.sqrt(1.0 - 1.0 / W ** 2)
+    bdir = rng.standard_normal((3, n))
+    bdir /= np.sqrt((bdir ** 2).sum(axis=0))
+    B = bdir * np.sqrt(rho * 10.0 ** rng.uniform(-4.0, 4.0, n))
+    E = _minus_v_cross_B(v, B) * (1.0 + noise * rng.standard_normal((3, n)))
+    return np.ascontiguousarray(np.concatenate([rho[None], v, p[None], B, E], axis=0))

@@ -184,3 +184,68 @@ def test_outflow_fill_is_zero_gradient(O, axis):
     # every other row of L vanishes (uniform fluid at rest, no fields)
     rest = [v for v in range(14) if v not in (8 + axis, 12)]
     assert np.all(np.abs(L[rest]) < 1e-12)
+
+
+# ------------------------------------------------------------------------------------------
+# con2prim on the hard tail and the second residual
+# ------------------------------------------------------------------------------------------
+EPS = np.finfo(float).eps
+
+
+def _backward_error(O, P, q, w2, W_true):
+    """A recovered state is judged by the conserved state it reproduces (the forward map prim2cons has its own closed-form
+    pins): max over D, S, tau of |q(w2) - q| / (|tau| + D + |S|), in units of eps W^2 -- the primitive set stores v, so
+    1 - v^2 ~ 1/W^2 carries a relative round-off of eps W^2 whatever the solver."""
+    q2 = O.prim2cons(P, w2, q[11])
+    scale = np.abs(q[4]) + q[0] + np.sqrt((q[1:4] ** 2).sum(0))
+    return (np.abs(q2[:5] - q[:5]).max(0) / scale) / (EPS * W_true ** 2)
+
+
+@pytest.mark.parametrize("gamma", [4.0 / 3.0, 5.0 / 3.0, 2.0])
+def test_con2prim_second_residual_alone(O, synth, gamma):
+    """The quartic in W (second residual) used from the first iteration (test hook oracle_set_c2p_switch(0)): closed form for
+    St = 0 (W = 1, Z = D + Gamma taut, p = (Gamma - 1) taut, rho = D) and round trip on random admissible states."""
+    P = O.make_params(model=0, gamma=gamma)
+    prev = O.set_c2p_switch(0)
+    try:
+        rng = np.random.default_rng(2)
+        n = 1000
+        D = 10 ** rng.uniform(-2, 2, n); taut = 10 ** rng.uniform(-3, 2, n)
+        B = rng.standard_normal((3, n)); E = rng.standard_normal((3, n))
+        q = np.zeros((14, n))
+        q[0] = D; q[1:4] = np.cross(E.T, B.T).T; q[4] = taut + 0.5 * ((E ** 2).sum(0) + (B ** 2).sum(0)); q[5:8] = B; q[8:11] = E
+        w, it, fl = O.con2prim(P, q)
+        assert not fl.any()
+        assert np.allclose(w[0], D, rtol=1e-13) and np.allclose(w[4], (gamma - 1) * taut, rtol=1e-12)
+        assert np.abs(w[1:4]).max() < 1e-12
+        n = 100000
+        w0 = synth.random_resistive_prims(n, seed=3, vmax=0.99)
+        q = O.prim2cons(P, w0)
+        w, it, fl = O.con2prim(P, q)
+        assert not fl.any() and it.max() <= 25
+        W = 1 / np.sqrt(1 - (w0[1:4] ** 2).sum(0))
+        assert _backward_error(O, P, q, w, W).max() < 64
+    finally:
+        O.set_c2p_switch(prev)
+
+
+@pytest.mark.parametrize("gamma", [4.0 / 3.0, 5.0 / 3.0, 2.0])
+def test_con2prim_hard_tail_never_fails(O, synth, gamma):
+    """W log-uniform up to 100, p/rho from 1e-8 to 1e4, B^2/rho up to 1e4, E within 1e-3 of -v x B, NO guess: every cell
+    is recovered, in a bounded number of iterations.  For Gamma = 4/3 and 5/3 the first residual (bracketed Newton in Z)
+    never needs more than 6 iterations; for Gamma = 2, W > 28 and p/rho > 600 it stalls (f'(Z) = 1/(2 W^2) + v^2/(2h) -> 0)
+    and, without the second residual, 1 cell in 2e5 is still not converged after 100 iterations; with the automatic switch
+    after 20 iterations every cell converges within 45.  Mutation caught: g_c2p_switch = 1000 (fall-back disabled)."""
+    P = O.make_params(model=0, gamma=gamma)
+    n = 200000
+    w0 = synth.stress_resistive_prims(n, seed=11)
+    q = O.prim2cons(P, w0)
+    w, it, fl = O.con2prim(P, q)
+    assert not fl.any(), np.bincount(fl)
+    assert it.max() <= 45
+    if gamma < 1.9:
+        assert it.max() <= 6
+    else:
+        assert (it > 20).sum() >= 1                       # the fall-back is exercised
+    W = 1 / np.sqrt(1 - (w0[1:4] ** 2).sum(0))
+    assert _backward_error(O, P, q, w, W).max() < 64
