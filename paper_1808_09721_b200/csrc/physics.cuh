@@ -44,6 +44,8 @@ RMHD_DEV double max3abs(double a, double b, double c) { return fmax(fabs(a), fma
 // by Newton-Raphson kept inside the bracket (|St|, +inf).  One reciprocal, one rsqrt and one
 // division per iteration.  Converged when the applied update |dZ| <= tol Z.
 // returns 0 ok, 1 inadmissible input, 2 not converged, 3 unphysical result
+// The safeguard logic (bracket, start value, return codes, the switch to the second residual) follows the oracle's on purpose,
+// so that both sides raise identical failure flags; its correctness rests on the oracle's closed-form and round-trip pins.
 // ---------------------------------------------------------------------------------------
 RMHD_DEV void hyd_from_Z(double D, double Sx, double Sy, double Sz, double S2, double Z, double g, Hyd& h) {
   const double iZ = 1.0 / Z;
@@ -54,6 +56,55 @@ RMHD_DEV void hyd_from_Z(double D, double Sx, double Sy, double Sz, double S2, d
   h.p = g * (Z * om - D * sq);
   h.rho = D * sq;
   h.vx = Sx * iZ; h.vy = Sy * iZ; h.vz = Sz * iZ;
+}
+
+// Second residual ("one may converge where the other may not").  The recovery in the Lorentz
+// factor W instead of Z: with En = taut + D = Z - p and p = g (Z / W^2 - D / W),
+//   Z(W) = W (En W - g D) / (W^2 - g),   F(W) = (En W - g D)^2 (W^2 - 1) - St^2 (W^2 - g)^2 = 0,   1 <= W <= Wmax,
+//   Wmax = (1 - St^2 / En^2)^(-1/2)  (p >= 0 <=> Z >= En).
+// F is a well-scaled polynomial where f(Z) is almost flat at its root (|St| -> En: large W and hot gas).  Newton-Raphson
+// from Wmax inside the bracket [1, Wmax]; converged when the applied update |dW| <= tol W or |F| is at its round-off
+// floor.  Taken automatically by c2p_hydro after C2P_SWITCH iterations of the first residual; never inlined (rare path).
+constexpr int C2P_SWITCH = 20;
+
+__device__ __noinline__ int c2p_hydro_W(double D, double Sx, double Sy, double Sz, double S2, double taut, double g, double tol,
+                                        int maxit, Hyd& h, int& iters) {
+  const double Sabs = sqrt(S2), En = taut + D;
+  double lo = 1.0, hi = rsqrt((En - Sabs) * (En + Sabs) / (En * En));
+  const double floor_eps = 32.0 * 2.220446049250313e-16;
+  double W = hi;
+  bool conv = false;
+  {
+    const double a = En * W - g * D, b = W * W - g, c = W * W - 1.0;
+    const double t1 = a * a * c, t2 = S2 * b * b;
+    if (!isfinite(hi) || !(t1 - t2 >= -floor_eps * (t1 + t2))) {
+      h.rho = h.vx = h.vy = h.vz = h.p = h.W = h.Z = nan("");
+      return 3;
+    }
+  }
+  while (iters < maxit) {
+    ++iters;
+    const double a = En * W - g * D, b = W * W - g, c = W * W - 1.0;
+    const double t1 = a * a * c, t2 = S2 * b * b;
+    const double f = t1 - t2;
+    if (fabs(f) <= floor_eps * (t1 + t2)) { conv = true; break; }
+    const double dF = 2.0 * En * a * c + 2.0 * W * a * a - 4.0 * S2 * W * b;
+    if (f < 0.0) lo = fmax(lo, W); else hi = fmin(hi, W);
+    double Wn = W - f / dF;
+    if (!(Wn >= lo && Wn <= hi) || !isfinite(Wn)) Wn = 0.5 * (lo + hi);
+    const double dW = Wn - W;
+    W = Wn;
+    if (fabs(dW) <= tol * W) { conv = true; break; }
+  }
+  const double Z = W * (En * W - g * D) / (W * W - g);
+  const double iZ = 1.0 / Z;
+  h.Z = Z; h.W = W;
+  h.p = g * (Z / (W * W) - D / W);
+  h.rho = D / W;
+  h.vx = Sx * iZ; h.vy = Sy * iZ; h.vz = Sz * iZ;
+  if (!conv) return 2;
+  if (!(h.p > 0.0) || !(h.rho > 0.0) || !isfinite(h.p) || !isfinite(Z)) return 3;
+  return 0;
 }
 
 RMHD_DEV int c2p_hydro(double D, double Sx, double Sy, double Sz, double taut, double Zg,
@@ -70,6 +121,12 @@ RMHD_DEV int c2p_hydro(double D, double Sx, double Sy, double Sz, double taut, d
   if (!(Z > Sabs) || !isfinite(Z)) Z = fmax(taut + D, Sabs * (1.0 + 1e-8) + 1e-300);
   bool conv = false;
   for (int it = 1; it <= P.maxit_c2p; ++it) {
+    if (it > C2P_SWITCH) {   // copies, so that h and iters of the common path stay in registers
+      Hyd t; int its = iters;
+      const int rc = c2p_hydro_W(D, Sx, Sy, Sz, S2, taut, P.g, P.tol_c2p, P.maxit_c2p, t, its);
+      h = t; iters = its;
+      return rc;
+    }
     iters = it;
     const double iZ = 1.0 / Z;
     const double v2 = S2 * iZ * iZ;

@@ -3,8 +3,14 @@ the same seeded inputs.  Run on the B200 box:  python -m pytest tests -m gpu
 
 Tolerances: per-cell algebra 1e-12..1e-13 relative; config
 runs use BASELINE.json's rel-L1 bounds (cfg1 1e-9, cfg2 1e-10, cfg3/4/5 1e-8), where
-rel-L1 = sum |q_gpu - q_oracle| / sum |q_oracle| over all conserved variables and cells.
+rel-L1 = sum |q_gpu - q_oracle| / sum |q_oracle| over all conserved variables and cells, AND, per conserved variable,
+sum |q_gpu - q_oracle| / max(sum |q_oracle|, N 1e-8) <= 1e-11: the global sum is dominated by tau and B,
+a defect in a small row (psi, phi, rho_charge) would not show in it.
 """
+import json
+import os
+import time
+
 import numpy as np
 import pytest
 
@@ -26,6 +32,45 @@ def B():
 
 def rel_l1(a, b):
     return np.abs(a - b).sum() / np.abs(b).sum()
+
+
+PER_VAR_TOL = 1e-11            # resistive model (measured: <= 5e-13)
+PER_VAR_TOL_TWO_FLUID = 1e-13  # x mu^2: two-fluid model, 1e-9 for |mu| = 100 (measured: <= 1.5e-10), see rel_l1_per_var
+
+
+def rel_l1_per_var(a, b, mu=None):
+    """per conserved variable, sum |a - b| / max(sum |b|, N 1e-8) (several rows are identically ~0 in cfg1 / cfg5).
+    Two-fluid model (18 rows, `mu` = max |mu_s|): the barred rows Dbar, Sbar, taubar are sums over species weighted by
+    mu_s = -+mu that cancel for a neutral pair plasma (they are identically ~0 in cfg4), so their round-off is mu eps times
+    the unbarred row: the denominator of row v in 5..9 is max(sum |b_v|, mu sum |b_{v-5}|).  That noise is fed back through the
+    source with omega_p^2 = sum mu_s^2 rho_s ~ mu^2 (A2 P:L445): the FMA / no-FMA difference of the two sides shows up at
+    ~mu^2 eps per step in E and psi, which is why the two-fluid bound is 1e-13 mu^2 (1e-9 for cfg4) and not 1e-11."""
+    n = b[0].size
+    out = []
+    for v in range(b.shape[0]):
+        den = max(np.abs(b[v]).sum(), n * 1e-8)
+        if mu is not None and 5 <= v <= 9:
+            den = max(den, mu * np.abs(b[v - 5]).sum())
+        out.append(np.abs(a[v] - b[v]).sum() / den)
+    return np.array(out)
+
+
+def check_state(name, q, qo, tol, per_var_tol=None, mu=None):
+    """Global rel-L1 <= the BASELINE.json bound and every variable's rel-L1 <= 1e-11 (two-fluid: 1e-9); the measured values go to
+    gpurun_out/parity_values.jsonl when RMHD_PARITY_LOG is set (they are quoted in BASELINE.md section 4)."""
+    two_fluid = qo.shape[0] == 18
+    if two_fluid and mu is None:
+        mu = 100.0
+    if per_var_tol is None:
+        per_var_tol = PER_VAR_TOL_TWO_FLUID * mu ** 2 if two_fluid else PER_VAR_TOL
+    g = float(rel_l1(q, qo)); pv = rel_l1_per_var(q, qo, mu if two_fluid else None)
+    if os.environ.get("RMHD_PARITY_LOG"):
+        os.makedirs("gpurun_out", exist_ok=True)
+        with open("gpurun_out/parity_values.jsonl", "a") as f:
+            f.write(json.dumps({"case": name, "rel_l1": g, "per_var_max": float(pv.max()), "per_var": [float(x) for x in pv]}) + "\n")
+    assert g <= tol, (name, g)
+    assert pv.max() <= per_var_tol, (name, int(pv.argmax()), pv)
+    return g, pv
 
 
 def run_gpu(B, cfg, nsteps=None, params_override=None):
@@ -78,7 +123,12 @@ def test_prim2cons_con2prim_batch_resistive(B, O, synth, n):
     assert not fl.any() and not flo.any()
     W2 = 1.0 / (1.0 - (w[1:4] ** 2).sum(0))
     cond = W2 * (1.0 + w[0] * (1 + 4 * w[4] / w[0]) / w[4])
-    assert (np.abs(w2[:5] - wo[:5]) / np.maximum(np.abs(wo[:5]), 1e-3) / cond).max() < 2e-12
+    err = (np.abs(w2[:5] - wo[:5]) / np.maximum(np.abs(wo[:5]), 1e-3) / cond).max()
+    if os.environ.get("RMHD_PARITY_LOG"):
+        os.makedirs("gpurun_out", exist_ok=True)
+        with open("gpurun_out/parity_values.jsonl", "a") as f:
+            f.write(json.dumps({"case": "con2prim batch n=%d" % n, "max_err_over_cond": float(err)}) + "\n")
+    assert err < 1e-12       # both sides stop at |dZ| <= 1e-13 Z with the update applied; measured 3.3e-13
     assert np.array_equal(w2[5:], wo[5:])
     assert np.abs(it - ito).max() <= 1
 
@@ -98,6 +148,41 @@ def test_prim2cons_con2prim_batch_two_fluid(B, O, synth):
     assert not fl.any() and not flo.any()
     assert (np.abs(w2 - wo) / np.maximum(np.abs(wo), 1e-2)).max() < 1e-9      # both sit at the same root
     assert rel_l1(w2, wo) < 1e-13
+
+
+@pytest.mark.parametrize("gamma", [4.0 / 3.0, 2.0])
+def test_con2prim_hard_tail_parity(B, O, synth, gamma):
+    """2^20 states with W up to 100, p/rho in [1e-8, 1e4], B^2/rho up to 1e4, E near -v x B,
+    no guess.  Both sides recover every cell; failure flags are identical; iteration counts agree to +-1 where the first
+    residual converges; for Gamma = 2 some cells take the second residual (quartic in W) on both sides.  The recovered
+    states are compared through the conserved state they reproduce (oracle prim2cons), in units of eps W^2."""
+    n = 1 << 20
+    w0 = synth.stress_resistive_prims(n, seed=11)
+    P, PO = B.make_params(model=0, gamma=gamma), O.make_params(model=0, gamma=gamma)
+    q = O.prim2cons(PO, w0)
+    w = np.empty((11, n)); it = np.zeros(n, np.int32); fl = np.zeros(n, np.int32)
+    B.rmhd_con2prim_batch(P, q, w, None, it, fl)
+    wo, ito, flo = O.con2prim(PO, q)
+    assert not fl.any() and not flo.any()
+    first = (it <= 20) & (ito <= 20)
+    # where the first residual is far from its round-off floor both sides take the same path; in the stalled tail (Gamma = 2, W > 28,
+    # p/rho > 600: the Newton update hovers around the tolerance) the counts differ by a few iterations on a handful of cells
+    if gamma < 1.9:
+        assert np.abs(it - ito).max() <= 1
+    assert (np.abs(it - ito) > 1).mean() < 0.02 and np.abs(it - ito).max() <= 45     # measured 0.8 %, max 32 (Gamma = 2: one side converges at the tolerance, the other stalls into the fall-back)
+    assert first.mean() > 0.9999 and it.max() <= 45
+    if gamma > 1.9:
+        assert (it > 20).sum() >= 1 and (ito > 20).sum() >= 1            # the fall-back runs on both sides (not on identical cells:
+        #                                                                  which cells stall at the tolerance is round-off dependent)
+    W = 1 / np.sqrt(1 - (w0[1:4] ** 2).sum(0))
+    eps = np.finfo(float).eps
+    scale = np.abs(q[4]) + q[0] + np.sqrt((q[1:4] ** 2).sum(0))
+    for ww in (w, wo):
+        q2 = O.prim2cons(PO, ww, q[11])
+        assert ((np.abs(q2[:5] - q[:5]).max(0) / scale) / (eps * W ** 2)).max() < 64
+    # element-wise where the problem is well conditioned (W < 10, 1e-4 < p/rho < 1e2, B^2 < rho: no large E x B to subtract)
+    good = (W < 10) & (w0[4] / w0[0] > 1e-4) & (w0[4] / w0[0] < 1e2) & ((w0[5:8] ** 2).sum(0) < w0[0])
+    assert (np.abs(w[:5] - wo[:5]) / np.maximum(np.abs(wo[:5]), 1e-300))[:, good].max() < 1e-9
 
 
 # ------------------------------------------------------------------------------------------
@@ -231,7 +316,7 @@ def test_config1_riemann_tube_full(B, O, synth):
     q, w, st = run_gpu(B, c)
     qo, wo, sto = run_oracle(O, c)
     assert st["n_failed"] == 0
-    assert rel_l1(q, qo) <= 1e-9, rel_l1(q, qo)
+    check_state("cfg1 128 cells x 128 steps", q, qo, 1e-9)
     assert st["hist_stage"].sum() == 2 * 128 * 128 and st["hist_c2p"].sum() == 128 * 128
     assert st["hist_stage"][0] == 0
 
@@ -241,7 +326,7 @@ def test_config3_shear_layer_reduced(B, O, synth):
     q, w, st = run_gpu(B, c)
     qo, wo, _ = run_oracle(O, c)
     assert st["n_failed"] == 0
-    assert rel_l1(q, qo) <= 1e-8, rel_l1(q, qo)
+    check_state("cfg3 96 x 128 x 60 steps", q, qo, 1e-8)
     assert rel_l1(w[:5], wo[:5]) <= 1e-8
 
 
@@ -253,7 +338,7 @@ def test_config3_shear_layer_full_size(B, O, synth):
     q, w, st = run_gpu(B, c)
     qo, wo, _ = run_oracle(O, c)
     assert st["n_failed"] == 0
-    assert rel_l1(q, qo) <= 1e-8, rel_l1(q, qo)
+    check_state("cfg3 512 x 512 x 200 steps", q, qo, 1e-8)
     assert rel_l1(w[:5], wo[:5]) <= 1e-8
 
 
@@ -262,7 +347,26 @@ def test_config5_blast_reduced(B, O, synth):
     q, w, st = run_gpu(B, c)
     qo, wo, _ = run_oracle(O, c)
     assert st["n_failed"] == 0
-    assert rel_l1(q, qo) <= 1e-8, rel_l1(q, qo)
+    check_state("cfg5 40^3 x 20 steps", q, qo, 1e-8)
+
+
+def test_config5_full_size_full_length(B, O, synth):
+    """BASELINE.json configs[4] as stated: 256^3, 20 steps, the WHOLE grid against the oracle, in the launch configuration
+    bench.py times.  Cost: 256^3 x 20 = 3.4e8 oracle zone-updates, about 6 minutes at the 9e5 zone-updates/s the oracle
+    reaches on the GPU box's 16 host threads, and about 25 GB of host memory (the oracle keeps 120 ghosted rows of
+    264^3 doubles).  RMHD_CFG5_FULL_N overrides the edge length (a smaller box for a quick look)."""
+    n = int(os.environ.get("RMHD_CFG5_FULL_N", "256"))
+    c = synth.config5(n=n, nsteps=20)
+    assert c["nsteps"] == 20
+    t0 = time.time()
+    q, w, st = run_gpu(B, c)
+    del w
+    qo, wo, sto = run_oracle(O, c)
+    del wo
+    assert st["n_failed"] == 0 and sto["n_failed"] == 0
+    g, pv = check_state("cfg5 %d^3 x 20 steps (whole grid)" % n, q, qo, 1e-8)
+    assert st["hist_stage"].sum() == 2 * n ** 3 * 20
+    print("cfg5 full: %.0f s, rel-L1 %.2e, per-variable max %.2e" % (time.time() - t0, g, pv.max()))
 
 
 def test_config5_full_size_sampled_against_oracle(B, O, synth):
@@ -306,9 +410,24 @@ def test_config4_two_fluid_reduced(B, O, synth):
     q, w, st = run_gpu(B, c)
     qo, wo, _ = run_oracle(O, c)
     assert st["n_failed"] == 0
-    assert rel_l1(q, qo) <= 1e-8, rel_l1(q, qo)
+    check_state("cfg4 64 x 48 x 50 steps", q, qo, 1e-8)
     assert rel_l1(w[:10], wo[:10]) <= 1e-8
     assert st["hist_stage"].sum() == 2 * 64 * 48 * 50
+
+
+def test_config4_full_size_full_length(B, O, synth):
+    """BASELINE.json configs[3] as stated: two-fluid, 1024 x 1024, 50 steps, the WHOLE grid against the oracle
+    (5.2e7 two-fluid oracle zone-updates: a few minutes on the GPU box's host threads)."""
+    c = synth.config4()
+    assert c["prims"].shape[1:] == (1, 1024, 1024) and c["nsteps"] == 50
+    t0 = time.time()
+    q, w, st = run_gpu(B, c)
+    qo, wo, sto = run_oracle(O, c)
+    assert st["n_failed"] == 0 and sto["n_failed"] == 0
+    g, pv = check_state("cfg4 1024 x 1024 x 50 steps (whole grid)", q, qo, 1e-8)
+    assert rel_l1(w[:10], wo[:10]) <= 1e-8
+    assert st["hist_stage"].sum() == 2 * 1024 * 1024 * 50
+    print("cfg4 full: %.0f s, rel-L1 %.2e, per-variable max %.2e" % (time.time() - t0, g, pv.max()))
 
 
 def test_config4_full_size_sampled_against_oracle(B, O, synth):
@@ -383,7 +502,7 @@ def test_ssp3_332_parity(B, O, synth, case, monkeypatch):
     q, w, st = run_gpu(B, c, nsteps=nsteps, params_override={"integrator": "ssp3"})
     qo, wo, _ = run_oracle(O, c, nsteps=nsteps, params_override={"integrator": "ssp3"})
     assert st["n_failed"] == 0
-    assert rel_l1(q, qo) <= tol, rel_l1(q, qo)
+    check_state("ssp3 " + case, q, qo, tol)
     ncell = int(np.prod(c["prims"].shape[1:]))
     assert st["hist_stage"].sum() == 3 * ncell * nsteps and st["hist_c2p"].sum() == ncell * nsteps
     # and it is a different scheme from SSP2(222)
@@ -415,7 +534,7 @@ def test_paper_setups_parity(B, O, synth, case, integrator):
     q, w, st = run_gpu(B, c)
     qo, wo, sto = run_oracle(O, c)
     assert st["n_failed"] == 0 and sto["n_failed"] == 0
-    assert rel_l1(q, qo) <= tol, rel_l1(q, qo)
+    check_state("paper %s %s" % (case, integrator), q, qo, tol, mu=max(abs(c["params"].get("mu_e", 0.0)), abs(c["params"].get("mu_p", 0.0))))
     nh = 5 if c["params"]["model"] == 0 else 10
     assert rel_l1(w[:nh], wo[:nh]) <= 10 * tol
 
@@ -429,7 +548,7 @@ def test_two_fluid_3d_blast_parity(B, O, synth, integrator, flux, monkeypatch):
     q, w, st = run_gpu(B, c)
     qo, wo, sto = run_oracle(O, c)
     assert st["n_failed"] == 0 and sto["n_failed"] == 0
-    assert rel_l1(q, qo) <= 1e-8, rel_l1(q, qo)
+    check_state("two-fluid 3-D blast %s %s" % (integrator, flux), q, qo, 1e-8)
     assert rel_l1(w[:10], wo[:10]) <= 1e-8
 
 
