@@ -128,6 +128,8 @@ class ClockSampler:
 def make_workload(name, synth):
     if name == "cfg5":
         return synth.config5()
+    if name == "cfg2":
+        return synth.config2()
     if name == "cfg3":
         return synth.config3()
     if name == "cfg1":
@@ -187,7 +189,7 @@ def time_oracle_one_thread(cfg, integrator="ssp2", m=48, budget_s=12.0):
     try:
         S = O.OracleSim(O.make_params(**p)); S.set_initial(w, rc)
         t0 = time.perf_counter(); done = 0
-        while done < 2 or (time.perf_counter() - t0 < budget_s / 3 and done < 8):
+        while done < 2 or (time.perf_counter() - t0 < min(1.0, budget_s / 3) and done < 4096):
             S.step(1); done += 1
         dt = time.perf_counter() - t0
         S.close()
@@ -230,6 +232,15 @@ def run_reference(args):
         return
     from paper_1808_09721_b200 import synth
     cfg = make_workload(args.workload, synth)
+    if args.workload == "cfg2":
+        v, cores, sample = cfg2_oracle_rate(cfg, 0, 1 << 16, budget_s=30.0)
+        base = {"value": v, "unit": CFG2_UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        print(json.dumps({"impl": "reference", "metric": CFG2_METRIC, "value": v, "unit": CFG2_UNIT, "n_gpus": args.gpus, "steps": args.steps,
+                          "warmup": 0, "ms_per_step": (1 << 16) / v * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                          "dtype": "f64", "data": "synthetic", "config": {"workload": cfg["name"] + " (oracle sample)", "sample": sample},
+                          "cpu_baseline": base, "e2e": {"value": v, "unit": CFG2_UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                          "gpu_launches": 0}))
+        return
     base, ms, done = time_oracle(cfg, synth, args.steps, min(args.warmup, 1), budget_s=120.0, integrator=args.integrator)
     line = {
         "impl": "reference", "metric": METRIC, "value": base["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": done,
@@ -266,6 +277,120 @@ def stage_flops(hist):
     its = (hist * np.arange(hist.size)).sum()
     n = hist.sum()
     return 420.0 * its + 150.0 * n
+
+
+# ---- BASELINE.json configs[1]: one batched implicit stage ------------------------------------------
+CFG2_METRIC, CFG2_UNIT = "fp64_cells_per_s_one_implicit_stage", "cells/s"
+CFG2_DOUBLES = 14 + 5 + 1 + 14 + 11        # R q_ex, guess (rho, v, p: B, E come with q_ex), sigma; W q*, prims  (+ 2 int32: iterations, flag)
+
+
+def cfg2_oracle_rate(cfg, threads, ncell, budget_s=10.0):
+    from oracle import oracle as O
+    prev = O.set_threads(0)
+    used = O.set_threads(threads) if threads else prev
+    try:
+        P = O.make_params(**cfg["params"])
+        w = np.ascontiguousarray(cfg["prims"][:, :ncell]); sg = np.ascontiguousarray(cfg["sigma_cell"][:ncell])
+        q_ex = O.prim2cons(P, w)
+        t0 = time.perf_counter(); done = 0
+        while done < 1 or time.perf_counter() - t0 < budget_s / 2:
+            O.stage_batch(P, q_ex, w, cfg["a_dt"], sg); done += 1
+        dt = time.perf_counter() - t0
+    finally:
+        O.set_threads(prev)
+    return ncell * done / dt, used, f"first {ncell} cells of the 2^20-cell batch, {done} stage solves in {dt:.1f} s"
+
+
+def run_cfg2(args, B, synth, torch, dist, dev, rank, world, local, hbm_peak, sm_max_mhz, peak_src, fp64_meas):
+    """2^20 independent resistive cells through rmhd_stage_batch (the implicit root-find is 55.3 % of the
+    paper's run time).  A step = one implicit stage over the whole batch, inputs and outputs resident in HBM."""
+    cfg = synth.config2()
+    n = cfg["prims"].shape[1]
+    P = B.make_params(**dict(cfg["params"], device=local))
+    w_d = torch.from_numpy(cfg["prims"]).to(dev); sg_d = torch.from_numpy(cfg["sigma_cell"]).to(dev)
+    qex_d = torch.empty((14, n), dtype=torch.float64, device=dev)
+    B.rmhd_prim2cons_batch(P, w_d, qex_d)
+    q_d = torch.empty_like(qex_d); wo_d = torch.empty_like(w_d)
+    it_d = torch.zeros(n, dtype=torch.int32, device=dev); fl_d = torch.zeros(n, dtype=torch.int32, device=dev)
+
+    def one():
+        B.rmhd_stage_batch(P, qex_d, w_d, cfg["a_dt"], q_d, wo_d, sg_d, it_d, fl_d)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    flush = torch.empty(160 * 1024 * 1024 // 8, dtype=torch.float64, device=dev)   # > 126 MB L2
+    for _ in range(args.warmup):
+        one()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    with ClockSampler(local) as clk:
+        for a, b in ev:
+            flush.fill_(1.0)                      # the batch (218 MB in + 210 MB out) exceeds L2, flushed all the same
+            a.record(); one(); b.record()
+        barrier()
+    ms_total = sum(a.elapsed_time(b) for a, b in ev)
+    value, ms_total = whole_job_rate(ms_total, n * args.steps, dist, dev)
+    its = it_d.cpu().numpy(); fl = fl_d.cpu().numpy()
+    hist = np.bincount(its, minlength=64).astype(np.float64)
+    ms = ms_total / args.steps
+    flops = stage_flops(hist)
+    t_hbm = (CFG2_DOUBLES * 8 + 8) * n / (hbm_peak * 1e9); t_alu = flops / (fp64_meas * 1e12)
+    bound = "hbm" if t_hbm >= t_alu else "alu"
+    roof = {"bound": bound, "kernel": "k_stage_batch_resistive",
+            "achieved": (flops / (ms * 1e-3) * 1e-12) if bound == "alu" else ((CFG2_DOUBLES * 8 + 8) * n / (ms * 1e-3) * 1e-9),
+            "peak": fp64_meas if bound == "alu" else hbm_peak, "unit": "TFLOP/s" if bound == "alu" else "GB/s",
+            "peak_source": "measured in this run: rmhd_probe_fp64 (DFMA chains on all SMs)" if bound == "alu" else peak_src + " (MEASURED_PEAKS.json hbm_gbs)",
+            "hbm_frac": t_hbm / (ms * 1e-3), "alu_frac": t_alu / (ms * 1e-3), "fp64_peak_measured_tflops": fp64_meas,
+            "fp64_peak_nominal_tflops": SM_COUNT * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 * 1e-12, "hbm_peak_gbs": hbm_peak,
+            "alg_bytes_per_cell": CFG2_DOUBLES * 8 + 8, "alg_flops_per_cell": flops / n, "avg_launch_ms": ms, "traffic": None,
+            "stage_iters_mean": float((hist * np.arange(hist.size)).sum() / n), "stage_iters_max": int(its.max()),
+            "stage_iters_hist": [int(x) for x in hist[:int(its.max()) + 1]]}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    cap = committed_ncu("cfg2", "stage")
+    if cap:
+        roof["traffic"] = cap.get("dram_bytes_per_launch", {}).get("stage_batch")
+        roof["fp64_pipe_busy_ncu"] = cap.get("fp64_pipe_busy", {}).get("stage_batch")
+        roof["ncu_traffic_committed"] = {"file": "profiles/ncu_traffic.json", "capture": cap.get("source"), "csrc_sha16": csrc_sha16()}
+    # end to end: host buffers in, host buffers out through the same C-ABI call (the library stages them on the device)
+    e2e = None
+    if rank == 0 or world > 1:
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        w_h, sg_h = pin(cfg["prims"]), pin(cfg["sigma_cell"])
+        qex_h = pin(qex_d.cpu().numpy())
+        q_h = torch.empty((14, n), dtype=torch.float64).pin_memory(); wo_h = torch.empty((11, n), dtype=torch.float64).pin_memory()
+        it_h = torch.zeros(n, dtype=torch.int32).pin_memory(); fl_h = torch.zeros(n, dtype=torch.int32).pin_memory()
+        e_steps = max(1, min(args.steps, 5))
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        B.rmhd_stage_batch(P, qex_h, w_h, cfg["a_dt"], q_h, wo_h, sg_h, it_h, fl_h)
+        barrier(); a.record()
+        for _ in range(e_steps):
+            B.rmhd_stage_batch(P, qex_h, w_h, cfg["a_dt"], q_h, wo_h, sg_h, it_h, fl_h)
+        b.record(); barrier()
+        e_rate, _ = whole_job_rate(a.elapsed_time(b), n * e_steps, dist, dev)
+        e2e = {"value": e_rate, "unit": CFG2_UNIT, "h2d_bytes_per_step": (14 + 11 + 1) * 8 * n, "d2h_bytes_per_step": (14 + 11 + 1) * 8 * n,
+               "steps": e_steps, "call": "rmhd_stage_batch(on_device = 0), pinned host buffers"}
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+    cpu_base = None
+    if world == 1 and not args.no_cpu_baseline:
+        vN, cores, sample = cfg2_oracle_rate(cfg, 0, 1 << 16)
+        v1, _, s1 = cfg2_oracle_rate(cfg, 1, 1 << 13)
+        cpu_base = {"value": vN, "unit": CFG2_UNIT, "cores": cores, "kind": "oracle", "sample": sample, "value_1thread": v1, "sample_1thread": s1}
+    line = {"metric": CFG2_METRIC, "value": value, "unit": CFG2_UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{cfg['name']}: {n} independent resistive cells, one implicit stage a = gamma x 1e-3, sigma log-uniform [1, 1e6]",
+                       "parallelism": "replicas only" if world > 1 else "1 gpu", "l2": "L2 flushed (160 MB fill) before every timed launch",
+                       "n_failed_cells": int((fl != 0).sum())},
+            "clocks": clk.summary(), "e2e": e2e, "gpu_launches": args.steps, "roofline": roof, "cpu_baseline": cpu_base}
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
 
 
 def run_ours(args):
