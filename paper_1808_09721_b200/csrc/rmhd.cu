@@ -41,6 +41,10 @@ struct rmhd_ctx {
   bool fused_flux;   // one-pass L(q) over all axes (flux_hm.cuh) when nx, ny > 1; RMHD_FLUX=split (see rmhd.h) forces the per-axis kernels
   int hm_ty;         // tile rows of the two-role flux kernel: 8 (one 16-warp CTA per SM) when ny >= 8, else 4 (two CTAs)
   int sm_count;
+  // small grids are launch-bound: one step's launch sequence is captured once into a CUDA graph and replayed (rmhd_step)
+  cudaGraphExec_t step_graph;
+  cudaStream_t cap_stream;
+  bool graph_failed;
   std::vector<EvRec> pending;
   std::vector<cudaEvent_t> ev_pool;
   double ms[KC_N];
@@ -331,6 +335,31 @@ int step_once_ssp3(rmhd_ctx* c) {
   return RMHD_OK;
 }
 
+int step_any(rmhd_ctx* c) {
+  if (c->p.integrator == RMHD_SSP3_332) return c->model == 0 ? step_once_ssp3<0>(c) : step_once_ssp3<1>(c);
+  return c->model == 0 ? step_once<0>(c) : step_once<1>(c);
+}
+
+constexpr size_t GRAPH_MAX_CELLS = (size_t)1 << 21;
+
+// Capture one step on a private stream (the caller's may be the legacy default stream, which cannot be captured) and
+// instantiate it; the graph is launched into the caller's stream.  Any failure leaves the plain launch path in force.
+void build_step_graph(rmhd_ctx* c) {
+  c->graph_failed = true;
+  if (!c->cap_stream && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return; }
+  cudaStream_t user = c->stream;
+  cudaGraph_t g = nullptr;
+  if (cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeRelaxed) != cudaSuccess) { cudaGetLastError(); return; }
+  c->stream = c->cap_stream;
+  const int rc = step_any(c);
+  c->stream = user;
+  const cudaError_t e = cudaStreamEndCapture(c->cap_stream, &g);
+  if (rc != RMHD_OK || e != cudaSuccess || !g) { if (g) cudaGraphDestroy(g); cudaGetLastError(); c->err.clear(); return; }
+  if (cudaGraphInstantiate(&c->step_graph, g, 0) != cudaSuccess) { c->step_graph = nullptr; cudaGetLastError(); }
+  else c->graph_failed = false;
+  cudaGraphDestroy(g);
+}
+
 int read_stats(rmhd_ctx* c) {
   CK(c, cudaMemcpyAsync(c->h_stats, c->d_stats, sizeof(Stats), cudaMemcpyDeviceToHost, c->stream));
   CK(c, cudaStreamSynchronize(c->stream));
@@ -389,6 +418,7 @@ int rmhd_create(const rmhd_params* p, rmhd_ctx** out) {
   c->sm_count = 148;
   for (int i = 0; i < KC_N; ++i) { c->ms[i] = 0.0; c->launches[i] = 0; }
   c->q = c->w = c->qs = c->L1 = c->L2 = c->Ps1 = c->Ps2 = c->A = nullptr; c->d_stats = nullptr; c->h_stats = nullptr;
+  c->step_graph = nullptr; c->cap_stream = nullptr; c->graph_failed = false;
   DeviceGuard dg(c->device);
   { int n = 0; if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, c->device) == cudaSuccess && n > 0) c->sm_count = n; }
   const size_t rows = (size_t)((p->integrator == RMHD_SSP3_332 ? 5 : 4) * c->nc + c->nh + 2 * c->ns);
@@ -418,6 +448,8 @@ void rmhd_destroy(rmhd_ctx* c) {
     if (c->stream || c->q) cudaStreamSynchronize(c->stream);
     for (auto& r : c->pending) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
     for (auto& e : c->ev_pool) cudaEventDestroy(e);
+    if (c->step_graph) cudaGraphExecDestroy(c->step_graph);
+    if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     if (c->q) cudaFree(c->q);
     if (c->d_stats) cudaFree(c->d_stats);
     if (c->h_stats) cudaFreeHost(c->h_stats);
@@ -482,10 +514,15 @@ int rmhd_set_cons(rmhd_ctx* c, const double* cons, const double* prim_guess, int
 int rmhd_step(rmhd_ctx* c, int nsteps) {
   if (!c || nsteps < 0) return RMHD_ERR_BAD_PARAM;
   DeviceGuard dg(c->device);
+  // Grids below GRAPH_MAX_CELLS are bound by launch latency (cfg1: 128 cells, 5 launches of a few microseconds each): the
+  // launch sequence of one step is the same every step (constant dt, fixed buffers), so it is captured once and replayed.
+  if (!c->profiling && nsteps >= 1 && c->N <= GRAPH_MAX_CELLS && !c->step_graph && !c->graph_failed) build_step_graph(c);
   for (int s = 0; s < nsteps; ++s) {
     int rc;
-    if (c->p.integrator == RMHD_SSP3_332) rc = c->model == 0 ? step_once_ssp3<0>(c) : step_once_ssp3<1>(c);
-    else rc = c->model == 0 ? step_once<0>(c) : step_once<1>(c);
+    if (c->step_graph && !c->profiling) {
+      CK(c, cudaGraphLaunch(c->step_graph, c->stream));
+      rc = RMHD_OK;
+    } else rc = step_any(c);
     if (rc) return rc;
     c->nsteps++;
   }
