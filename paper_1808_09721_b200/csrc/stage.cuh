@@ -186,8 +186,9 @@ namespace rmhd {
 //            tau_s = c_s tbar + d_s (tau - (E^2+B^2)/2),   v_s = S_s / Z_s
 // with m_s = mu_s D_s, m2_s = mu_s^2 D_s (constants of the stage), Kq = sum m2_s, rhoc = sum m_s,
 // J = sum m_s v_s, U = sum m2_s v_s, wp2 = sum m2_s sqrt(1-v_s^2), rho0 = (Kq rhoc - J.U)/wp2.
-// Jacobian by exact forward-mode tangents, one direction at a time (all in registers); Z_e, Z_p
-// eliminated (dG_s/dZ_t = 0 for s != t), leaving a 7x7 system solved by Gaussian elimination
+// Jacobian by exact forward-mode tangents, one direction at a time (all in registers); Z_e, Z_p are
+// eliminated in closed form inside the species tangent (G_s depends on one Z only and on x through
+// v_s . dS_s and dtau_s; see t_stage_iter), leaving a 7x7 system solved by Gaussian elimination
 // in the order (Sbar, tbar, E): the pivots are 1 + a eta wp2 k > 0 and 1 + a^2 k Kq/(..) > 0
 // (k = sum m_s c_s / Z_s), so no pivoting is needed.
 // ---------------------------------------------------------------------------------------
@@ -260,17 +261,6 @@ RMHD_DEV void t_stage_init(TStage& s, const double* qe, const double* wg, double
   }
 }
 
-// tangent of one species' kinematics: inputs (dS, dZ, dtau_s) -> dv, dsq, dG
-RMHD_DEV void t_kin_tan(const TKin& k, double Z, double D, double g, double dSx, double dSy, double dSz, double dZ, double dts,
-                        double* dv, double& dsq, double& dG) {
-  dv[0] = (dSx - k.vx * dZ) * k.iZ;
-  dv[1] = (dSy - k.vy * dZ) * k.iZ;
-  dv[2] = (dSz - k.vz * dZ) * k.iZ;
-  const double dom = -2.0 * (k.vx * dv[0] + k.vy * dv[1] + k.vz * dv[2]);
-  dsq = 0.5 * dom * k.W;
-  dG = dZ - g * (dZ * k.om + Z * dom - D * dsq) - dts;
-}
-
 struct TAgg { double J[3], U[3], wp2, iw, rho0; };
 
 // tangent of the seven F rows given the species tangents and the direct (dSb, dtb, dE) parts
@@ -327,53 +317,58 @@ RMHD_DEV void t_stage_iter(TStage& s, const DevPar& P) {
     F[6] = s.E[2] - s.Eex[2] + s.a * A.J[2];
   }
   const double zero3[3] = {0.0, 0.0, 0.0};
-  // ---- Z_s directions: dF/dZ_s (7 each), dG_s/dZ_s
-  double FZ[2][7], rGZ[2];
+  // ---- Z_s eliminated in closed form.  With dZ_s = 0:  dG_s = gam_s (v_s . dS_s) - dtau_s, gam_s = g (2 - D_s W_s / Z_s);
+  // dG_s/dZ_s = f'(Z_s) = 1 - g (1 + v^2 - D W v^2 / Z) (con2prim's derivative).  The Newton condition G_s + dG_s = 0 gives
+  //   dZ_s = -(G_s + gam_s v_s . dS_s - dtau_s) / f'_s,    dv_s = (dS_s - v_s dZ_s) / Z_s,    dsq_s = -W_s (v_s . dv_s),
+  // i.e. dv_s is affine in (dS_s, dtau_s): the constant part (from G_s) goes to the right-hand side, the linear part
+  // into the 7 x 7 matrix.  Same Newton step as a Schur complement on the 9 x 9 system, without its Z rows and columns.
+  double gam[2], rfp[2];
 #pragma unroll
   for (int q = 0; q < 2; ++q) {
-    double dv[2][3] = {{0, 0, 0}, {0, 0, 0}}, dsq[2] = {0, 0}, dG;
-    t_kin_tan(k[q], s.Z[q], s.D[q], P.g, 0.0, 0.0, 0.0, 1.0, 0.0, dv[q], dsq[q], dG);
-    t_F_tan(s, A, dv, dsq, zero3, 0.0, zero3, FZ[q]);
-    rGZ[q] = 1.0 / dG;
+    const double v2 = 1.0 - k[q].om;
+    gam[q] = P.g * (2.0 - s.D[q] * k[q].W * k[q].iZ);
+    rfp[q] = 1.0 / (1.0 - P.g * (1.0 + v2 - s.D[q] * k[q].W * v2 * k[q].iZ));
   }
-  // ---- x directions; M = dF/dx - sum_s dF/dZ_s (dG_s/dx) / (dG_s/dZ_s);  GX[s][j] = dG_s/dx_j
-  double M[7][7], GX[2][7];
+  auto species_tan = [&](int q, double dSx, double dSy, double dSz, double dts, double G0, double* dv, double& dsq) {
+    const double vdS = k[q].vx * dSx + k[q].vy * dSy + k[q].vz * dSz;
+    const double mdZ = (G0 + gam[q] * vdS - dts) * rfp[q];          // = -dZ_s
+    dv[0] = (dSx + k[q].vx * mdZ) * k[q].iZ;
+    dv[1] = (dSy + k[q].vy * mdZ) * k[q].iZ;
+    dv[2] = (dSz + k[q].vz * mdZ) * k[q].iZ;
+    dsq = -(k[q].vx * dv[0] + k[q].vy * dv[1] + k[q].vz * dv[2]) * k[q].W;
+  };
+  double b[7];
+  {   // right-hand side: -(F + dF/dv . dv0), dv0 = the change of v_s when Z_s alone takes its Newton correction
+    double dv[2][3], dsq[2], dF[7];
+#pragma unroll
+    for (int q = 0; q < 2; ++q) species_tan(q, 0.0, 0.0, 0.0, 0.0, G[q], dv[q], dsq[q]);
+    t_F_tan(s, A, dv, dsq, zero3, 0.0, zero3, dF);
+#pragma unroll
+    for (int i = 0; i < 7; ++i) b[i] = -(F[i] + dF[i]);
+  }
+  double M[7][7];
 #pragma unroll
   for (int j = 0; j < 7; ++j) {
-    double dF[7], dGs[2];
-    if (j == 3) {            // taubar: only tau_s changes
-#pragma unroll
-      for (int i = 0; i < 7; ++i) dF[i] = i == 3 ? 1.0 : 0.0;
-      dGs[0] = -s.c[0]; dGs[1] = -s.c[1];
-    } else {
-      double dSb[3] = {0, 0, 0}, dE[3] = {0, 0, 0}, dSt[3] = {0, 0, 0}, dtaut = 0.0, cS = 0.0;
-      if (j < 3) { dSb[j] = 1.0; cS = 1.0; }
-      else {
-        const int e = j - 4;
-        dE[e] = 1.0;
-        // d(S - E x B)/dE_e = -(e_e x B)
-        if (e == 0) { dSt[1] = s.Bz; dSt[2] = -s.By; }
-        if (e == 1) { dSt[0] = -s.Bz; dSt[2] = s.Bx; }
-        if (e == 2) { dSt[0] = s.By; dSt[1] = -s.Bx; }
-        dtaut = -s.E[e];
-      }
-      double dv[2][3], dsq[2];
-#pragma unroll
-      for (int q = 0; q < 2; ++q)
-        t_kin_tan(k[q], s.Z[q], s.D[q], P.g, s.c[q] * cS * dSb[0] + s.d[q] * dSt[0], s.c[q] * cS * dSb[1] + s.d[q] * dSt[1],
-                  s.c[q] * cS * dSb[2] + s.d[q] * dSt[2], 0.0, s.d[q] * dtaut, dv[q], dsq[q], dGs[q]);
-      t_F_tan(s, A, dv, dsq, dSb, 0.0, dE, dF);
+    double dSb[3] = {0, 0, 0}, dE[3] = {0, 0, 0}, dSt[3] = {0, 0, 0}, dtb = 0.0, dtaut = 0.0;
+    if (j < 3) dSb[j] = 1.0;
+    else if (j == 3) dtb = 1.0;
+    else {
+      const int e = j - 4;
+      dE[e] = 1.0;
+      // d(S - E x B)/dE_e = B x e_e
+      if (e == 0) { dSt[1] = s.Bz; dSt[2] = -s.By; }
+      if (e == 1) { dSt[0] = -s.Bz; dSt[2] = s.Bx; }
+      if (e == 2) { dSt[0] = s.By; dSt[1] = -s.Bx; }
+      dtaut = -s.E[e];
     }
-    const double w0 = dGs[0] * rGZ[0], w1 = dGs[1] * rGZ[1];
-    GX[0][j] = dGs[0]; GX[1][j] = dGs[1];
+    double dv[2][3], dsq[2], dF[7];
 #pragma unroll
-    for (int i = 0; i < 7; ++i) M[i][j] = dF[i] - FZ[0][i] * w0 - FZ[1][i] * w1;
-  }
-  double b[7];
-  {
-    const double w0 = G[0] * rGZ[0], w1 = G[1] * rGZ[1];
+    for (int q = 0; q < 2; ++q)
+      species_tan(q, s.c[q] * dSb[0] + s.d[q] * dSt[0], s.c[q] * dSb[1] + s.d[q] * dSt[1], s.c[q] * dSb[2] + s.d[q] * dSt[2],
+                  s.c[q] * dtb + s.d[q] * dtaut, 0.0, dv[q], dsq[q]);
+    t_F_tan(s, A, dv, dsq, dSb, dtb, dE, dF);
 #pragma unroll
-    for (int i = 0; i < 7; ++i) b[i] = -(F[i] - FZ[0][i] * w0 - FZ[1][i] * w1);
+    for (int i = 0; i < 7; ++i) M[i][j] = dF[i];
   }
   // ---- Gaussian elimination, no pivoting (see header comment)
 #pragma unroll
@@ -396,12 +391,16 @@ RMHD_DEV void t_stage_iter(TStage& s, const DevPar& P) {
     dx[i] = t / M[i][i];
   }
   double dZ[2];
+  {
+    // dS_s, dtau_s of the solved update:  dSt = B x dE,  dtaut = -E . dE
+    const double tx = s.By * dx[6] - s.Bz * dx[5], ty = s.Bz * dx[4] - s.Bx * dx[6], tz = s.Bx * dx[5] - s.By * dx[4];
+    const double dtaut = -(s.E[0] * dx[4] + s.E[1] * dx[5] + s.E[2] * dx[6]);
 #pragma unroll
-  for (int q = 0; q < 2; ++q) {
-    double t = G[q];
-#pragma unroll
-    for (int j = 0; j < 7; ++j) t += GX[q][j] * dx[j];
-    dZ[q] = -t * rGZ[q];
+    for (int q = 0; q < 2; ++q) {
+      const double vdS = k[q].vx * (s.c[q] * dx[0] + s.d[q] * tx) + k[q].vy * (s.c[q] * dx[1] + s.d[q] * ty) +
+                         k[q].vz * (s.c[q] * dx[2] + s.d[q] * tz);
+      dZ[q] = -(G[q] + gam[q] * vdS - (s.c[q] * dx[3] + s.d[q] * dtaut)) * rfp[q];
+    }
   }
   s.iters++;
   double sum = dZ[0] + dZ[1];
