@@ -21,8 +21,12 @@
 // sheet; ideal limit; two-fluid Langmuir frequency; general IMEX stepper and
 // SSP3(332) (Table 3): order conditions, implicit stability function, Shu-Osher
 // RK3 recomposition through eval_L, telegraph-mode closed form, Table 2 through the general
-// stepper against the SSP2(222) path, second-order convergence.  Full configs 1,3,4,5
-// have no printed reference values in the paper: "parity unpinned" beyond those pins.
+// stepper against the SSP2(222) path, second-order convergence.  tests/test_oracle_pins_r2.py:
+// two-fluid source rows with friction on a charged, moving state (hand values; rho_0 of reading G2),
+// Gauss-law initial charge density, zero-gradient outflow fill, the second con2prim residual alone
+// and the hard tail (W up to 100, p/rho up to 1e4) -- each checked against a named mutation.
+// Full configs 1,3,4,5 have no printed reference values in the paper: "parity unpinned" beyond
+// those pins; no function of this file is without a pin.
 //
 // Build: g++ -O2 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/build.py).
 // -ffp-contract=off: the paper itself switches FMA off; also needed for the
