@@ -56,10 +56,10 @@ def csrc_sha16():
 
 
 def committed_ncu(workload, integrator):
-    """profiles/ncu_traffic.json: DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) and FP64 pipe
+    """profiles/ncu_traffic.txt: DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) and FP64 pipe
     utilisation from one committed `ncu --set full` capture, keyed by workload/integrator; None if the capture was taken
     on other kernel sources."""
-    path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.txt")
     if not os.path.exists(path):
         return None
     with open(path) as f:
@@ -354,7 +354,7 @@ def run_cfg2(args, B, synth, torch, dist, dev, rank, world, local, hbm_peak, sm_
     if cap:
         roof["traffic"] = cap.get("dram_bytes_per_launch", {}).get("stage_batch")
         roof["fp64_pipe_busy_ncu"] = cap.get("fp64_pipe_busy", {}).get("stage_batch")
-        roof["ncu_traffic_committed"] = {"file": "profiles/ncu_traffic.json", "capture": cap.get("source"), "csrc_sha16": csrc_sha16()}
+        roof["ncu_traffic_committed"] = {"file": "profiles/ncu_traffic.txt", "capture": cap.get("source"), "csrc_sha16": csrc_sha16()}
     # end to end: host buffers in, host buffers out through the same C-ABI call (the library stages them on the device)
     e2e = None
     if rank == 0 or world > 1:
@@ -514,7 +514,7 @@ def run_ours(args):
     roof["traffic"] = None
     if cap and dom in cap.get("dram_bytes_per_launch", {}):
         roof["traffic"] = cap["dram_bytes_per_launch"][dom]
-        roof["ncu_traffic_committed"] = {"file": "profiles/ncu_traffic.json", "capture": cap.get("source"), "csrc_sha16": csrc_sha16()}
+        roof["ncu_traffic_committed"] = {"file": "profiles/ncu_traffic.txt", "capture": cap.get("source"), "csrc_sha16": csrc_sha16()}
         if dom in cap.get("fp64_pipe_busy", {}):
             roof["fp64_pipe_busy_ncu"] = cap["fp64_pipe_busy"][dom]
     # Whole step: the bytes THIS build's launches move (sum over the launches of a step of the per-launch figures above),
