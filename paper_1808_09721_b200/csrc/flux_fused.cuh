@@ -188,4 +188,160 @@ RMHD_DEV void prefetch_rows(const FluxComb& cb, size_t N, unsigned id, ROW row) 
   }
 }
 
+// G = g^+ + g^- (= 2 x the numerical flux) of every conserved row from the NF reconstructed fields of one face
+template <int MODEL, int K>
+RMHD_DEV void assemble_G(const double* o, double* G) {
+  using FS = FSet<MODEL>;
+  constexpr int a = (K + 1) % 3, b = (K + 2) % 3;
+#pragma unroll
+  for (int h = 0; h < FS::NHV; ++h) G[FS::hv(h)] = o[h] + o[FS::NHV + h];
+  const double* p = o + 2 * FS::NHV;
+  G[FS::IB + a] = p[0] - p[4];
+  G[FS::IE + b] = -(p[0] + p[4]);
+  G[FS::IB + b] = p[1] + p[5];
+  G[FS::IE + a] = p[1] - p[5];
+  G[FS::IB + K] = p[2] + p[6];
+  G[FS::IPHI] = p[2] - p[6];
+  G[FS::IE + K] = p[3] + p[7];
+  G[FS::IPSI] = p[3] - p[7];
+}
+// the NF reconstructions of one face from shared memory.  Field f lives at p + f*fs, cells are st apart,
+// p[0] is the cell two to the left of the face ("+": cells 0,1,2 ; "-": cells 3,2,1).  8 chains in flight.
+template <int MODEL, int F0 = 0>
+RMHD_DEV void face_recon(const double* p, int fs, int st, double* o) {
+  constexpr int NF = FSet<MODEL>::NF;
+  constexpr int G = NF - F0 >= 8 ? 8 : NF - F0;
+  double a[G], b[G], c[G];
+#pragma unroll
+  for (int g = 0; g < G; ++g) {
+    const double* pf = p + (F0 + g) * fs;
+    if (field_is_plus<MODEL>(F0 + g)) { a[g] = pf[0]; b[g] = pf[st]; c[g] = pf[2 * st]; }
+    else { a[g] = pf[3 * st]; b[g] = pf[2 * st]; c[g] = pf[st]; }
+  }
+  weno3_batch<G, true>(a, b, c, o + F0);
+  if constexpr (F0 + G < NF) face_recon<MODEL, F0 + G>(p, fs, st, o);
+}
+
+// =======================================================================================
+// a4: L(q) along ONE axis (every 1-D grid; y and z of RMHD_FLUX=split use k_flux_march).  Flux vector + Lax-Friedrichs
+// split (eq 12, alpha = 1) + WENO3 + face flux + divergence, one CTA per tile, the stencil staged through shared memory,
+// with the paired Maxwell fields of the one-pass kernel (NF = 20 / 28 reconstructions per face instead of 28 / 36):
+//   phase 1  every cell of the tile + 2 halo cells per side: load q, w (boundary index map = virtual ghost zones, a6),
+//            the NF unscaled fields g+- of the axis -> smem
+//   phase 2  one thread per face: NF WENO3 reconstructions, G = 2 x the face flux of every row (registers, then smem
+//            aliased onto the field buffer)
+//   phase 3  one thread per cell: L (=|+=) -(G_{i+1/2} - G_{i-1/2}) / (2 dx)
+// AXIS 0: lanes run along the sweep axis (x): tile 64 cells x 4 rows.
+// AXIS 1,2: lanes run along x, the sweep axis is strided: tile 32 (x) x 8 (sweep).
+// =======================================================================================
+template <int AXIS> struct Tile { static constexpr int TS = 8, TO = 32; };
+template <> struct Tile<0> { static constexpr int TS = 64, TO = 4; };
+constexpr int FLUX_THREADS = 288;
+constexpr int FLUX_PREFETCH_CTAS = 148 * 2 + 24;   // resident CTAs (2 per SM) plus a margin
+
+template <int MODEL, int AXIS>
+constexpr size_t flux_smem_bytes() { return sizeof(double) * FSet<MODEL>::NF * (Tile<AXIS>::TS + 4) * Tile<AXIS>::TO; }
+
+template <int MODEL, int AXIS>
+__global__ void __launch_bounds__(FLUX_THREADS, 2) k_flux(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, size_t N,
+                                                          int nx, int ny, int nz, int bc, double inv_dx, int accumulate, DevPar P) {
+  constexpr int NC = Dim<MODEL>::NC, NH = Dim<MODEL>::NH, NF = FSet<MODEL>::NF;
+  constexpr int TS = Tile<AXIS>::TS, TO = Tile<AXIS>::TO;
+  constexpr int CS = (TS + 4) * TO;   // cells incl. halo
+  constexpr int FS = (TS + 1) * TO;   // faces
+  static_assert(FS <= FLUX_THREADS && TS * TO <= FLUX_THREADS, "one pass per phase");
+  static_assert(NC * FS <= NF * CS, "G aliases the field buffer");
+  extern __shared__ double sm[];      // fields [NF][CS];  later G [NC][FS]
+  const int tid = threadIdx.x;
+  const int ns = AXIS == 0 ? nx : (AXIS == 1 ? ny : nz);
+  const int no = AXIS == 0 ? ny * nz : nx;
+  const int o0 = blockIdx.x * TO;
+  // a 1-D grid (AXIS 0, one row) lays the TO tile rows along x: row o covers cells s0 + o TS ... (all threads busy)
+  const bool rows_x = AXIS == 0 && no == 1;
+  const int s0 = rows_x ? blockIdx.y * (TS * TO) : blockIdx.y * TS;
+  const int third = blockIdx.z;
+
+  // ---- L2 prefetch of the tile that the CTA about one wave behind this one will stage (AXIS 0 only)
+  if (AXIS == 0 && !rows_x) {
+    const long long lin = (long long)blockIdx.x + (long long)gridDim.x * blockIdx.y + FLUX_PREFETCH_CTAS;
+    if (lin < (long long)gridDim.x * gridDim.y && tid < CS) {
+      const int pbx = (int)(lin % gridDim.x), pby = (int)(lin / gridDim.x);
+      const int c = pby * TS - 2 + tid % (TS + 4), oo = pbx * TO + tid / (TS + 4);
+      if (c < ns + 2 && oo < no) {
+        const size_t idx = (size_t)oo * nx + bc_map(c, ns, bc);
+#pragma unroll
+        for (int v = 0; v < NC; ++v) prefetch_l2(qin.r[v] + idx);
+#pragma unroll
+        for (int v = 0; v < NH; ++v) prefetch_l2(win.r[v] + idx);
+      }
+    }
+  }
+  // ---- phase 1
+  for (int item = tid; item < CS; item += FLUX_THREADS) {
+    int sh, o;
+    if (AXIS == 0) { sh = item % (TS + 4); o = item / (TS + 4); } else { o = item % TO; sh = item / TO; }
+    const int c = s0 - 2 + sh + (rows_x ? o * TS : 0);
+    const int oo = rows_x ? 0 : o0 + o;
+    if (c < ns + 2 && oo < no) {
+      const int cm = bc_map(c, ns, bc);
+      size_t idx;
+      if (AXIS == 0) idx = (size_t)oo * nx + cm;
+      else if (AXIS == 1) idx = ((size_t)third * ny + cm) * nx + oo;
+      else idx = ((size_t)cm * ny + third) * nx + oo;
+      double ql[NC], wl[NH], g[NF];
+#pragma unroll
+      for (int v = 0; v < NC; ++v) ql[v] = __ldg(qin.r[v] + idx);
+#pragma unroll
+      for (int v = 0; v < NH; ++v) wl[v] = __ldg(win.r[v] + idx);
+      Com<MODEL> cm_;
+      cell_common(ql, wl, P, cm_);
+      cell_fields<MODEL, AXIS>(ql, wl, cm_, P, g);
+#pragma unroll
+      for (int f = 0; f < NF; ++f) sm[f * CS + item] = g[f];
+    }
+  }
+  __syncthreads();
+
+  // ---- phase 2: face fs is the left face of tile cell fs (halo coordinate fs + 2)
+  double G[NC];
+  const bool has_face = tid < FS;
+  if (has_face) {
+    int fs, o, st;
+    if (AXIS == 0) { fs = tid % (TS + 1); o = tid / (TS + 1); st = 1; }
+    else { o = tid % TO; fs = tid / TO; st = TO; }
+    const int base = AXIS == 0 ? o * (TS + 4) + fs : fs * TO + o;   // halo coordinate fs
+    double rec[NF];
+    face_recon<MODEL>(sm + base, CS, st, rec);
+    assemble_G<MODEL, AXIS>(rec, G);
+  }
+  __syncthreads();
+  if (has_face) {
+#pragma unroll
+    for (int v = 0; v < NC; ++v) sm[v * FS + tid] = G[v];
+  }
+  __syncthreads();
+
+  // ---- phase 3
+  if (tid < TS * TO) {
+    int s, o, fi, st;
+    if (AXIS == 0) { s = tid % TS; o = tid / TS; fi = o * (TS + 1) + s; st = 1; }
+    else { o = tid % TO; s = tid / TO; fi = s * TO + o; st = TO; }
+    const int c = s0 + s + (rows_x ? o * TS : 0);
+    const int oo = rows_x ? 0 : o0 + o;
+    if (c < ns && oo < no) {
+      size_t idx;
+      if (AXIS == 0) idx = (size_t)oo * nx + c;
+      else if (AXIS == 1) idx = ((size_t)third * ny + c) * nx + oo;
+      else idx = ((size_t)c * ny + third) * nx + oo;
+      const double hid = 0.5 * inv_dx;
+#pragma unroll
+      for (int v = 0; v < NC; ++v) {
+        const double val = -(sm[v * FS + fi + st] - sm[v * FS + fi]) * hid;
+        double* dst = L + (size_t)v * N + idx;
+        *dst = accumulate ? *dst + val : val;
+      }
+    }
+  }
+}
+
 }  // namespace rmhd

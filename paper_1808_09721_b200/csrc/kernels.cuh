@@ -422,124 +422,6 @@ __global__ void __launch_bounds__(128) k_stage_batch_two_fluid(const double* __r
 }
 
 // =======================================================================================
-// a4: L(q) along one axis.  Flux vector + Lax-Friedrichs split (eq 12, alpha = 1) + WENO3 +
-// face flux + divergence, one CTA per tile, the stencil staged through shared memory:
-//   phase 1  every cell of the tile + 2 halo cells per side: load q, w (boundary index map =
-//            virtual ghost zones, a6), flux vector, f+- = (f +- q)/2  -> smem
-//   phase 2  one thread per face: 2 x NC WENO3 reconstructions -> F (registers, then smem
-//            aliased onto the f+- buffer)
-//   phase 3  one thread per cell: L (=|+=) -(F_{i+1/2} - F_{i-1/2}) / dx
-// AXIS 0: lanes run along the sweep axis (x): tile 64 cells x 4 rows.
-// AXIS 1,2: lanes run along x, the sweep axis is strided: tile 32 (x) x 8 (sweep).
-// =======================================================================================
-template <int AXIS> struct Tile { static constexpr int TS = 8, TO = 32; };
-template <> struct Tile<0> { static constexpr int TS = 64, TO = 4; };
-constexpr int FLUX_THREADS = 288;
-constexpr int FLUX_PREFETCH_CTAS = 148 * 2 + 24;   // resident CTAs (2 per SM) plus a margin
-
-template <int MODEL, int AXIS>
-constexpr size_t flux_smem_bytes() { return sizeof(double) * 2 * Dim<MODEL>::NC * (Tile<AXIS>::TS + 4) * Tile<AXIS>::TO; }
-
-template <int MODEL, int AXIS>
-__global__ void __launch_bounds__(FLUX_THREADS, 2) k_flux(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, size_t N,
-                                                          int nx, int ny, int nz, int bc, double inv_dx, int accumulate, DevPar P) {
-  constexpr int NC = Dim<MODEL>::NC, NH = Dim<MODEL>::NH;
-  constexpr int TS = Tile<AXIS>::TS, TO = Tile<AXIS>::TO;
-  constexpr int CS = (TS + 4) * TO;   // cells incl. halo
-  constexpr int FS = (TS + 1) * TO;   // faces
-  static_assert(FS <= FLUX_THREADS && TS * TO <= FLUX_THREADS, "one pass per phase");
-  extern __shared__ double sm[];      // f+ [NC][CS], f- [NC][CS];  later F [NC][FS]
-  const int tid = threadIdx.x;
-  const int ns = AXIS == 0 ? nx : (AXIS == 1 ? ny : nz);
-  const int no = AXIS == 0 ? ny * nz : nx;
-  const int o0 = blockIdx.x * TO;
-  // a 1-D grid (AXIS 0, one row) lays the TO tile rows along x: row o covers cells s0 + o TS ... (all threads busy)
-  const bool rows_x = AXIS == 0 && no == 1;
-  const int s0 = rows_x ? blockIdx.y * (TS * TO) : blockIdx.y * TS;
-  const int third = blockIdx.z;
-
-  // ---- L2 prefetch of the tile that the CTA about one wave behind this one will stage (AXIS 0 only)
-  if (AXIS == 0 && !rows_x) {
-    const long long lin = (long long)blockIdx.x + (long long)gridDim.x * blockIdx.y + FLUX_PREFETCH_CTAS;
-    if (lin < (long long)gridDim.x * gridDim.y && tid < CS) {
-      const int pbx = (int)(lin % gridDim.x), pby = (int)(lin / gridDim.x);
-      const int c = pby * TS - 2 + tid % (TS + 4), oo = pbx * TO + tid / (TS + 4);
-      if (c < ns + 2 && oo < no) {
-        const size_t idx = (size_t)oo * nx + bc_map(c, ns, bc);
-#pragma unroll
-        for (int v = 0; v < NC; ++v) prefetch_l2(qin.r[v] + idx);
-#pragma unroll
-        for (int v = 0; v < NH; ++v) prefetch_l2(win.r[v] + idx);
-      }
-    }
-  }
-  // ---- phase 1
-  for (int item = tid; item < CS; item += FLUX_THREADS) {
-    int sh, o;
-    if (AXIS == 0) { sh = item % (TS + 4); o = item / (TS + 4); } else { o = item % TO; sh = item / TO; }
-    const int c = s0 - 2 + sh + (rows_x ? o * TS : 0);
-    const int oo = rows_x ? 0 : o0 + o;
-    if (c < ns + 2 && oo < no) {
-      const int cm = bc_map(c, ns, bc);
-      size_t idx;
-      if (AXIS == 0) idx = (size_t)oo * nx + cm;
-      else if (AXIS == 1) idx = ((size_t)third * ny + cm) * nx + oo;
-      else idx = ((size_t)cm * ny + third) * nx + oo;
-      double ql[NC], wl[NH], f[NC];
-#pragma unroll
-      for (int v = 0; v < NC; ++v) ql[v] = __ldg(qin.r[v] + idx);
-#pragma unroll
-      for (int v = 0; v < NH; ++v) wl[v] = __ldg(win.r[v] + idx);
-      if (MODEL == 0) r_flux<AXIS>(ql, wl, P.sigma, P, f); else t_flux<AXIS>(ql, wl, P, f);
-#pragma unroll
-      for (int v = 0; v < NC; ++v) {
-        sm[v * CS + item] = 0.5 * (f[v] + ql[v]);
-        sm[(NC + v) * CS + item] = 0.5 * (f[v] - ql[v]);
-      }
-    }
-  }
-  __syncthreads();
-
-  // ---- phase 2: face fs is the left face of tile cell fs (halo coordinate fs + 2)
-  double F[NC];
-  const bool has_face = tid < FS;
-  if (has_face) {
-    int fs, o, st;
-    if (AXIS == 0) { fs = tid % (TS + 1); o = tid / (TS + 1); st = 1; }
-    else { o = tid % TO; fs = tid / TO; st = TO; }
-    const int base = AXIS == 0 ? o * (TS + 4) + fs : fs * TO + o;   // halo coordinate fs
-    weno_faces<NC>(sm + base, sm + NC * CS + base, CS, st, F);
-  }
-  __syncthreads();
-  if (has_face) {
-#pragma unroll
-    for (int v = 0; v < NC; ++v) sm[v * FS + tid] = F[v];
-  }
-  __syncthreads();
-
-  // ---- phase 3
-  if (tid < TS * TO) {
-    int s, o, fi, st;
-    if (AXIS == 0) { s = tid % TS; o = tid / TS; fi = o * (TS + 1) + s; st = 1; }
-    else { o = tid % TO; s = tid / TO; fi = s * TO + o; st = TO; }
-    const int c = s0 + s + (rows_x ? o * TS : 0);
-    const int oo = rows_x ? 0 : o0 + o;
-    if (c < ns && oo < no) {
-      size_t idx;
-      if (AXIS == 0) idx = (size_t)oo * nx + c;
-      else if (AXIS == 1) idx = ((size_t)third * ny + c) * nx + oo;
-      else idx = ((size_t)c * ny + third) * nx + oo;
-#pragma unroll
-      for (int v = 0; v < NC; ++v) {
-        const double val = -(sm[v * FS + fi + st] - sm[v * FS + fi]) * inv_dx;
-        double* dst = L + (size_t)v * N + idx;
-        *dst = accumulate ? *dst + val : val;
-      }
-    }
-  }
-}
-
-// =======================================================================================
 // a4, axes 1 and 2 (sweep axis strided in memory): MARCHING kernel.  Lanes run along x, so the
 // stencil never crosses lanes: each thread owns one (x, other) column and marches along the
 // sweep axis over a segment, keeping the 3-cell f+ / 2-cell f- window of its column in shared
