@@ -86,3 +86,31 @@ def test_product_path_never_imports_the_oracle():
     assert "#include \"" not in osrc            # the oracle includes no project header
     for f in ("oracle.py", "build.py"):
         assert "paper_1808_09721_b200" not in open(os.path.join(ROOT, "oracle", f)).read()
+
+
+def test_binding_rejects_buffers_of_the_wrong_size_before_the_call(B):
+    """Marshalling checks (binding.py `_expect`): a buffer with the wrong row or cell count would be an out-of-bounds device
+    access inside the library; the binding refuses it before any pointer crosses the ABI (no GPU needed)."""
+    p = B.make_params(nx=8, sigma=1.0)
+    q = np.zeros((14, 4)); w = np.zeros((11, 4))
+    with pytest.raises(ValueError):
+        B.rmhd_stage_batch(p, q, np.zeros((10, 4)), 1e-3, q.copy(), w.copy())          # prim_guess one row short
+    with pytest.raises(ValueError):
+        B.rmhd_stage_batch(p, q, w, 1e-3, np.zeros((14, 3)), w.copy())                 # q_out one cell short
+    with pytest.raises(ValueError):
+        B.rmhd_stage_batch(p, q, w, 1e-3, q.copy(), w.copy(), sigma_cell=np.zeros(5))
+    with pytest.raises(ValueError):
+        B.rmhd_prim2cons_batch(p, w, np.zeros((18, 4)))                                 # two-fluid sized output, resistive model
+    with pytest.raises(ValueError):
+        B.rmhd_con2prim_batch(p, q, w, fail=np.zeros(3, np.int32))
+    with pytest.raises(ValueError):
+        B.rmhd_con2prim_batch(p, q.astype(np.float32), w)                               # wrong dtype
+
+
+def test_the_one_environment_switch_is_documented(B):
+    """include/rmhd.h names every environment variable the library reads."""
+    src = open(os.path.join(ROOT, "paper_1808_09721_b200", "csrc", "rmhd.cu")).read()
+    envs = set(re.findall(r'getenv\("([A-Z_0-9]+)"\)', src))
+    assert envs == {"RMHD_FLUX"}
+    hdr = open(os.path.join(ROOT, "include", "rmhd.h")).read()
+    assert "RMHD_FLUX=split" in hdr and "test_ssp3_332_parity[blast_3d_split]" in hdr

@@ -473,6 +473,48 @@ def test_unphysical_input_is_reported(B, synth):
     sim.close()
 
 
+def test_graph_replay_equals_plain_launches_bitwise(B, synth):
+    """rmhd_step replays one captured step as a CUDA graph on grids of up to 2^21 cells; profiling mode uses plain launches.
+    Same kernels, same arguments: the states must be bitwise equal (1-D, 2-D and 3-D, both integrators)."""
+    for c, kw in ((synth.config1(nx=100), {}), (synth.config3(nx=64, ny=40, nsteps=6), {}), (synth.config5(n=24, nsteps=6), {}),
+                  (synth.config5(n=24, nsteps=6), {"integrator": "ssp3"}), (synth.config4(nx=40, ny=24, nsteps=6), {})):
+        p = dict(c["params"]); p.update(kw)
+        a = B.Rmhd(**p); a.set_initial(np.ascontiguousarray(c["prims"]), c.get("rho_charge"))
+        a.step(1); a.step(5)
+        qa, wa = a.get_state(); sa = a.stats(); a.close()
+        b = B.Rmhd(**p); b.set_initial(np.ascontiguousarray(c["prims"]), c.get("rho_charge"))
+        B.rmhd_set_profiling(b.ctx, True)
+        b.step(6)
+        qb, wb = b.get_state(); sb = b.stats(); b.close()
+        assert np.array_equal(qa, qb) and np.array_equal(wa, wb)
+        assert np.array_equal(sa["hist_stage"], sb["hist_stage"]) and np.array_equal(sa["hist_c2p"], sb["hist_c2p"])
+
+
+def test_degenerate_calls(B, synth):
+    """nsteps = 0 is a no-op; an empty batch is accepted; a grid of 2^31 cells is refused before anything is allocated; set_cons
+    resets the statistics so that its return code is its own."""
+    c = synth.config5(n=16, nsteps=1)
+    sim = B.Rmhd(**c["params"]); sim.set_initial(c["prims"])
+    q0, _ = sim.get_state()
+    assert sim.step(0) == B.RMHD_OK and sim.time == 0.0
+    q1, _ = sim.get_state()
+    assert np.array_equal(q0, q1)
+    sim.step(2)
+    assert sim.stats()["hist_stage"].sum() == 2 * 2 * 16 ** 3
+    assert sim.set_cons(q0) == 0
+    st = sim.stats()
+    assert st["hist_stage"].sum() == 0 and st["hist_c2p"].sum() == 16 ** 3 and st["n_failed"] == 0
+    assert abs(sim.time - 2 * sim.dt) < 1e-18          # the step counter is untouched
+    sim.close()
+    P = B.make_params(model=0, gamma=G43, sigma=1.0)
+    e = np.empty((14, 0)); w = np.empty((11, 0))
+    B.rmhd_stage_batch(P, e, w, 1e-3, e.copy(), w.copy())
+    B.rmhd_con2prim_batch(P, e, w.copy())
+    with pytest.raises(B.RmhdError) as ex:
+        B.Rmhd(model=0, nx=2048, ny=2048, nz=512, sigma=1.0)
+    assert ex.value.code == B.RMHD_ERR_BAD_PARAM
+
+
 def test_set_cons_get_state_round_trip_and_device_buffers(B, O, synth):
     import torch
     c = synth.config3(nx=32, ny=24, nsteps=3)
