@@ -143,6 +143,42 @@ int rmhd_prim2cons_batch(const rmhd_params* p, long long ncells, const double* p
 int rmhd_con2prim_batch(const rmhd_params* p, long long ncells, const double* cons, const double* prim_guess,
                         double* prims, int* iters, int* fail, int on_device);
 
+/* ---- L(q) without any allocation ----------------------------------------------------------------------
+ * For callers who cannot let this library allocate device memory.  Two kinds of program are meant: one that
+ * has handed the whole card to a memory pool of its own (a cudaMalloc made behind that pool's back can fail
+ * with out-of-memory while the pool still has room, and the pool's bookkeeping never learns of it), and one
+ * whose time loop must not stall (cudaFree synchronises the whole device and cudaMalloc may: every other
+ * stream on the card waits).  rmhd_create and the on_device = 0 batch calls above do allocate; this call does not.
+ *
+ * What it computes: the same L(q) = -sum_d dF^d/dx_d as rmhd_flux_divergence (eq 12 + WENO3) of a
+ * conserved state the CALLER holds, in two steps: primitive recovery (no initial guess), then the flux
+ * kernels.  cons and Lout are DEVICE pointers on device p->device, [14|18][nz][ny][nx], owned by the caller, 8-byte
+ * aligned, not overlapping.  Of *p the model, grid, domain, bc, gamma, tol_c2p, max_iter_c2p, device and stream are
+ * read (sigma, eta, mu_e, mu_p are only range-checked; integrator and cfl are ignored; RMHD_FLUX is honoured
+ * as in rmhd_create).  n_failed (HOST pointer, may be NULL) receives the number of cells whose recovery failed.
+ *
+ * Where the scratch lives: the recovered hydro primitives ([5|10] rows) and the failure counters are neither input
+ * nor output, and sit in ONE fixed array inside the library image, 20 MiB + 4 KiB.  Every GPU on which the library
+ * is used holds that array from the moment the library's code is loaded there until the process exits, whether or
+ * not this call is ever made.  Its capacity is the limit of this call: nx*ny*nz <= RMHD_STATIC_MAX_CELLS (2^18,
+ * e.g. 512 x 512 or 64^3) for either model; a larger grid is refused with RMHD_ERR_BAD_PARAM and a message
+ * that names the limit (rmhd_last_error(NULL)), before anything is launched.
+ *
+ * First call on a device: it looks up the array's device address (cudaGetSymbolAddress, with that device
+ * current) and remembers it; make that first call before any stream capture begins.  Later calls only launch
+ * kernels, copy about 1 KB of counters back and synchronise p->stream; no call uses cudaMalloc, cudaFree or a
+ * library routine that allocates (on the error paths the message is a host-side std::string).
+ *
+ * Sharing: there is one array per GPU, not one per call or per stream.  It keeps what the previous call wrote;
+ * the counters are cleared at the start of every call, the primitive rows are overwritten before they are read.
+ * Two calls whose kernels can run at the same time on one GPU (two streams, two host threads) race on it and
+ * both results are garbage: serialise them.  The call returns only when L is complete, so back-to-back calls from
+ * one thread are safe.
+ * Returns: OK; BAD_PARAM (null pointer, bad parameters, grid beyond the limit); CUDA (no device: there is no CPU
+ * fallback; launch failure); NONCONVERGED if any cell's recovery failed (L is then not valid near those cells). */
+#define RMHD_STATIC_MAX_CELLS 262144
+int rmhd_flux_divergence_static(const rmhd_params* p, const double* cons, double* Lout, long long* n_failed);
+
 /* ---- roofline denominators measured by the library's own probe kernels (SURVEY.md section 7 step 0:
  * MEASURED_PEAKS.json holds no FP64 figure, so the FP64 roofline peak is this probe's) ------------- */
 /* FP64 FMA chain on all SMs: returns achieved TFLOP/s (2 flop per DFMA) in *tflops. */

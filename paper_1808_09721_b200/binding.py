@@ -28,8 +28,9 @@ EXPORTS = (
     "rmhd_create", "rmhd_set_initial", "rmhd_set_cons", "rmhd_step", "rmhd_get_state", "rmhd_flux_divergence",
     "rmhd_get_stats", "rmhd_set_profiling", "rmhd_get_kernel_times", "rmhd_dt", "rmhd_time", "rmhd_last_error",
     "rmhd_destroy", "rmhd_stage_batch", "rmhd_prim2cons_batch", "rmhd_con2prim_batch", "rmhd_probe_fp64",
-    "rmhd_probe_hbm",
+    "rmhd_probe_hbm", "rmhd_flux_divergence_static",
 )
+RMHD_STATIC_MAX_CELLS = 262144   # include/rmhd.h: capacity of the library's fixed scratch array (rmhd_flux_divergence_static)
 
 
 class RmhdError(RuntimeError):
@@ -116,6 +117,7 @@ def lib():
     L.rmhd_con2prim_batch.argtypes = [pp, C.c_longlong, vp, vp, vp, vp, vp, C.c_int]
     L.rmhd_probe_fp64.argtypes = [C.c_int, vp, _dp]
     L.rmhd_probe_hbm.argtypes = [C.c_int, vp, C.c_longlong, _dp]
+    L.rmhd_flux_divergence_static.argtypes = [pp, vp, vp, _lp]
     _lib = L
     return L
 
@@ -260,6 +262,25 @@ def rmhd_con2prim_batch(params, cons, prims, prim_guess=None, iters=None, fail=N
     a, d1 = _ptr(cons); g, d2 = _ptr(prim_guess); w, d3 = _ptr(prims)
     it, d4 = _ptr(iters, np.int32); fl, d5 = _ptr(fail, np.int32)
     _check(lib().rmhd_con2prim_batch(C.byref(params), n, a, g, w, it, fl, _same_side(d1, d2, d3, d4, d5)))
+
+
+def rmhd_flux_divergence_static(params, cons, Lout, check=True):
+    """L(q) of a conserved state held by the caller, for callers that cannot let the library allocate device memory (their
+    own pool owns the card, or their loop cannot take the device-wide stall of cudaMalloc / cudaFree).  `cons` and `Lout`
+    are CUDA tensors [14|18][nz][ny][nx] on params.device; the grid may have at most RMHD_STATIC_MAX_CELLS cells, because
+    the scratch is one fixed array inside the library, shared by all calls on that GPU: do not overlap two calls.
+    Returns (code, n_failed); with check=True a non-zero code raises instead."""
+    n = params.nx * params.ny * params.nz
+    nc = NCONS[params.model]
+    _expect(cons, nc, n, "cons", params.device); _expect(Lout, nc, n, "Lout", params.device)
+    a, d1 = _ptr(cons); b, d2 = _ptr(Lout)
+    if d1 != 1 or d2 != 1:
+        raise ValueError("rmhd_flux_divergence_static takes device buffers only (CUDA tensors)")
+    nf = C.c_longlong(0)
+    rc = lib().rmhd_flux_divergence_static(C.byref(params), a, b, C.byref(nf))
+    if check:
+        _check(rc)
+    return rc, nf.value
 
 
 def rmhd_probe_fp64(device=0, stream=None):

@@ -5,6 +5,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -778,3 +779,103 @@ int rmhd_probe_hbm(int device, void* stream, long long bytes, double* gbs) {
 }
 
 }  // extern "C"
+
+// ---- L(q) of a caller-supplied conserved state with no allocation (rmhd_flux_divergence_static, rmhd.h) -------------
+// The flux kernels read the hydro primitives next to the conserved rows, and the recovery kernel that produces them counts
+// its failures in a statistics block: two pieces of device memory that are neither input nor output of "cons in, L out".
+// Everywhere else in this file they come from cudaMalloc (rmhd_create).  Here they live in one fixed array that is part of
+// the library image, for the programs that must not let a library allocate: a host application that has given the card's
+// memory to a pool of its own (an allocation made behind the pool's back can fail while the pool still has room, and the
+// pool's accounting never sees it), or a time loop that cannot afford the device-wide synchronisation cudaFree performs and
+// cudaMalloc may perform (it serialises every other stream on the card).
+namespace {
+
+constexpr size_t STATIC_MAX_CELLS = RMHD_STATIC_MAX_CELLS;
+constexpr size_t STATIC_STATS_BYTES = 4096;   // the Stats block, padded so that the primitive rows behind it start on a 256-byte boundary
+constexpr size_t STATIC_BYTES = STATIC_STATS_BYTES + sizeof(double) * T_NH * STATIC_MAX_CELLS;   // 20 MiB + 4 KiB: 10 rows (two-fluid) of 2^18 cells
+static_assert(sizeof(Stats) <= STATIC_STATS_BYTES, "statistics block outgrew its slot");
+
+// Resident on every GPU that loads librmhd.so, from module load to process exit.  Device code may name it; in host code the
+// name is only a handle for cudaGetSymbolAddress, never an address a kernel can use.
+static __device__ __align__(256) unsigned char g_static_scratch[STATIC_BYTES];
+
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mu;
+unsigned char* g_static_addr[STATIC_MAX_DEVICES];   // the array's address on each device, looked up on that device's first call
+
+// p->device must be the current device
+int static_scratch_address(int device, unsigned char** out) {
+  if (device < 0 || device >= STATIC_MAX_DEVICES) { g_create_error = "rmhd_flux_divergence_static: device ordinal beyond 63"; return RMHD_ERR_BAD_PARAM; }
+  std::lock_guard<std::mutex> lk(g_static_mu);
+  if (!g_static_addr[device]) {
+    void* a = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&a, g_static_scratch);
+    if (e != cudaSuccess || !a) return fail_cuda(nullptr, e, "cudaGetSymbolAddress(g_static_scratch)");
+    g_static_addr[device] = (unsigned char*)a;
+  }
+  *out = g_static_addr[device];
+  return RMHD_OK;
+}
+
+// the counters are accumulated with atomics and the array keeps whatever the previous call left: every call starts here
+__global__ void k_static_reset(Stats* st) {
+  for (int b = threadIdx.x; b < NBINS; b += blockDim.x) { st->hist_stage[b] = 0ULL; st->hist_c2p[b] = 0ULL; }
+  if (threadIdx.x == 0) { st->n_failed = 0ULL; st->first_failed = LLONG_MAX; st->n_bad_input = 0ULL; }
+}
+
+template <int MODEL>
+int flux_divergence_static(rmhd_ctx* c, const double* cons, double* w, Stats* st, double* Lout) {
+  k_static_reset<<<1, NBINS, 0, c->stream>>>(st);
+  CK(c, cudaGetLastError());
+  k_con2prim<MODEL><<<blocks_for(c->N, 256), 256, 0, c->stream>>>(cons, nullptr, c->N, w, c->N, nullptr, nullptr, nullptr, c->N, c->P, st);
+  CK(c, cudaGetLastError());
+  return launch_flux<MODEL>(c, cons, nullptr, false, w, Lout);
+}
+
+}  // namespace
+
+extern "C" int rmhd_flux_divergence_static(const rmhd_params* p, const double* cons, double* Lout, long long* n_failed) {
+  if (n_failed) *n_failed = 0;
+  if (!p || !cons || !Lout) { g_create_error = "rmhd_flux_divergence_static: null argument"; return RMHD_ERR_BAD_PARAM; }
+  if (p->nx < 1 || p->ny < 1 || p->nz < 1) { g_create_error = "rmhd_flux_divergence_static: bad grid size"; return RMHD_ERR_BAD_PARAM; }
+  const unsigned long long cells = (unsigned long long)p->nx * (unsigned long long)p->ny * (unsigned long long)p->nz;
+  if (cells > STATIC_MAX_CELLS) {
+    char buf[400];
+    snprintf(buf, sizeof buf, "rmhd_flux_divergence_static: %d x %d x %d = %llu cells exceed RMHD_STATIC_MAX_CELLS = %llu, the capacity of the "
+             "library's fixed scratch array; larger grids go through rmhd_create + rmhd_set_cons + rmhd_flux_divergence",
+             p->nx, p->ny, p->nz, cells, (unsigned long long)STATIC_MAX_CELLS);
+    g_create_error = buf;
+    return RMHD_ERR_BAD_PARAM;
+  }
+  for (int d = 0; d < 3; ++d) if (p->bc[d] != RMHD_BC_OUTFLOW && p->bc[d] != RMHD_BC_PERIODIC) { g_create_error = "rmhd_flux_divergence_static: bad boundary condition"; return RMHD_ERR_BAD_PARAM; }
+  rmhd_ctx c{};   // lives on this stack frame only: the launch helpers read the grid, the parameters and the stream from it
+  int rc = batch_prologue(p, (long long)cells, c.P);   // parameter checks; RMHD_ERR_CUDA without a device (no CPU fallback)
+  if (rc) return rc;
+  c.p = *p; c.model = p->model;
+  c.nc = p->model == 0 ? R_NC : T_NC; c.nh = p->model == 0 ? R_NH : T_NH; c.ns = p->model == 0 ? R_NS : T_NS; c.np = p->model == 0 ? 11 : 16;
+  c.n[0] = p->nx; c.n[1] = p->ny; c.n[2] = p->nz; c.N = (size_t)cells;
+  const double lo[3] = {p->xmin, p->ymin, p->zmin}, hi[3] = {p->xmax, p->ymax, p->zmax};
+  for (int d = 0; d < 3; ++d) {
+    c.dx[d] = (hi[d] - lo[d]) / c.n[d];
+    if (c.n[d] > 1 && !(c.dx[d] > 0.0)) { g_create_error = "rmhd_flux_divergence_static: empty domain"; return RMHD_ERR_BAD_PARAM; }
+  }
+  c.device = p->device; c.stream = (cudaStream_t)p->stream;
+  { const char* e = getenv("RMHD_FLUX"); c.fused_flux = !(e && strcmp(e, "split") == 0); }   // the same switch rmhd_create reads (rmhd.h)
+  c.hm_ty = p->ny >= 8 ? 8 : 4;
+  c.sm_count = 148;
+  DeviceGuard dg(c.device);
+  { int n = 0; if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, c.device) == cudaSuccess && n > 0) c.sm_count = n; }
+  unsigned char* scratch = nullptr;
+  if ((rc = static_scratch_address(c.device, &scratch))) return rc;
+  Stats* st = (Stats*)scratch;
+  double* w = (double*)(scratch + STATIC_STATS_BYTES);
+  rc = c.model == 0 ? flux_divergence_static<0>(&c, cons, w, st, Lout) : flux_divergence_static<1>(&c, cons, w, st, Lout);
+  if (rc) { g_create_error = c.err; return rc; }
+  Stats h;   // the call returns when L is complete, like rmhd_flux_divergence: one 1 KB read-back and a stream synchronisation
+  cudaError_t e = cudaMemcpyAsync(&h, st, sizeof(Stats), cudaMemcpyDeviceToHost, c.stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c.stream);
+  if (e != cudaSuccess) return fail_cuda(nullptr, e, "rmhd_flux_divergence_static");
+  if (n_failed) *n_failed = (long long)h.n_failed;
+  if (h.n_failed) { g_create_error = "rmhd_flux_divergence_static: primitive recovery failed in some cells (count in *n_failed); L is not valid near them"; return RMHD_ERR_NONCONVERGED; }
+  return RMHD_OK;
+}
