@@ -125,10 +125,19 @@ int c2p_hydro_W(double D, const double* St, double taut, double gam, double tol,
   const double floor_eps = 32.0 * std::numeric_limits<double>::epsilon();
   double lo = 1.0, hi = 1.0 / std::sqrt((E - Sabs) * (E + Sabs) / (E * E));
   double dF, mag;
-  if (!std::isfinite(hi) || !(F(hi, dF, mag) >= -floor_eps * mag)) return 3;          // no root with p >= 0
   double W = hi;
   bool conv = false;
-  while (iters < maxit) {
+  // Near-static state, Wmax - 1 <= 1e-9 (|St| / E below about 4e-5): W^2 - 1 is then known to a few ulps of 1 only (it
+  // rounds to exactly 0 once |St| / E < 1e-8, and F(Wmax) = -St^2 (1-g)^2 would read "no root"), so the quartic cannot
+  // be iterated.  Its root is taken in closed form instead: W^2 - 1 = v^2 = St^2 / Z^2 with Z = Z(W = 1) = (E - g D) / (1 - g),
+  // W = sqrt(1 + v^2) = 1 + v^2 / 2; the neglected terms are O(v^4) <= 4e-18.  (Reading G4.)
+  if (hi - 1.0 <= 1e-9) {
+    const double Z1 = (E - g * D) / (1.0 - g);
+    W = 1.0 + 0.5 * S2 / (Z1 * Z1);
+    ++iters;
+    conv = true;
+  } else if (!std::isfinite(hi) || !(F(hi, dF, mag) >= -floor_eps * mag)) return 3;   // no root with p >= 0
+  while (!conv && iters < maxit) {
     ++iters;
     const double f = F(W, dF, mag);
     if (std::fabs(f) <= floor_eps * mag) { conv = true; break; }

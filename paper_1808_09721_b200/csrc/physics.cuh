@@ -74,7 +74,14 @@ __device__ __noinline__ int c2p_hydro_W(double D, double Sx, double Sy, double S
   const double floor_eps = 32.0 * 2.220446049250313e-16;
   double W = hi;
   bool conv = false;
-  {
+  if (hi - 1.0 <= 1e-9) {
+    // near-static state: W^2 - 1 carries only a few ulps of 1 (exactly 0 once |St| / En < 1e-8, where F(Wmax) would read
+    // "no root"); the root in closed form, W = 1 + v^2 / 2 with v^2 = St^2 / Z(W = 1)^2, error O(v^4) <= 4e-18
+    const double Z1 = (En - g * D) / (1.0 - g);
+    W = 1.0 + 0.5 * S2 / (Z1 * Z1);
+    ++iters;
+    conv = true;
+  } else {
     const double a = En * W - g * D, b = W * W - g, c = W * W - 1.0;
     const double t1 = a * a * c, t2 = S2 * b * b;
     if (!isfinite(hi) || !(t1 - t2 >= -floor_eps * (t1 + t2))) {
@@ -82,7 +89,7 @@ __device__ __noinline__ int c2p_hydro_W(double D, double Sx, double Sy, double S
       return 3;
     }
   }
-  while (iters < maxit) {
+  while (!conv && iters < maxit) {
     ++iters;
     const double a = En * W - g * D, b = W * W - g, c = W * W - 1.0;
     const double t1 = a * a * c, t2 = S2 * b * b;

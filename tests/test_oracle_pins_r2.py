@@ -249,3 +249,36 @@ def test_con2prim_hard_tail_never_fails(O, synth, gamma):
         assert (it > 20).sum() >= 1                       # the fall-back is exercised
     W = 1 / np.sqrt(1 - (w0[1:4] ** 2).sum(0))
     assert _backward_error(O, P, q, w, W).max() < 64
+
+
+@pytest.mark.parametrize("gamma", [4.0 / 3.0, 2.0])
+def test_con2prim_second_residual_near_static_states(O, gamma):
+    """Second residual alone (oracle_set_c2p_switch(0)) on states that barely move, |v| from 1e-12 to 1e-4 with E = -v x B exactly
+    cancelled out of S (B = E = 0): Wmax - 1 = O(v^2) is below one ulp of 1 for |v| < 1e-8, W^2 - 1 rounds to 0 and the quartic reads
+    F(Wmax) = -St^2 (1 - g)^2 < 0.  The recovery must return the state all the same (closed-form limit W = 1 + v^2 / 2), not
+    flag 3.  Expected values are the primitives the state was built from (eq 2-4, written out here).
+    Mutation this catches: dropping the near-static branch flags every cell with |v| < 1e-8 as unphysical."""
+    P = O.make_params(model=0, gamma=gamma)
+    rng = np.random.default_rng(5)
+    n = 4000
+    rho = 10 ** rng.uniform(-2, 2, n); p = 10 ** rng.uniform(-3, 2, n)
+    vabs = 10 ** rng.uniform(-12, -4, n)
+    d = rng.standard_normal((3, n)); d /= np.sqrt((d ** 2).sum(0))
+    v = vabs * d
+    W = 1.0 / np.sqrt(1.0 - (v ** 2).sum(0))
+    h = 1.0 + gamma / (gamma - 1.0) * p / rho
+    Z = rho * h * W ** 2
+    q = np.zeros((14, n))
+    q[0] = rho * W; q[1:4] = Z * v; q[4] = Z - p - rho * W
+    prev = O.set_c2p_switch(0)
+    try:
+        w, it, fl = O.con2prim(P, q)
+    finally:
+        O.set_c2p_switch(prev)
+    assert not fl.any(), (int((fl != 0).sum()), float(vabs[fl != 0].max()))
+    assert np.abs(w[0] / rho - 1).max() < 1e-13 and np.abs(w[4] / p - 1).max() < 1e-10     # p = g (Z - D) cancels for cold gas
+    assert (np.abs(w[1:4] - v).max(0) / vabs).max() < 1e-12
+    assert it.max() <= 12
+    # and the default path (first residual, then the second) agrees with it
+    w1, _, fl1 = O.con2prim(P, q)
+    assert not fl1.any() and np.abs(w1[:5] - w[:5]).max() < 1e-9 * np.abs(w[:5]).max()
