@@ -134,20 +134,14 @@ def make_workload(name, synth):
         return synth.config3()
     if name == "cfg1":
         return synth.config1()
-    if name == "cfg3_big":          # same recipe at 4096^2 = 2^24 cells (kernel studies; not a BASELINE config)
-        return synth.config3(nx=4096, ny=4096)
     if name == "cfg4":
         return synth.config4()
-    if name == "cfg5_small":
-        return synth.config5(n=64)
     if name == "bw17":              # the paper's profile-table workload: 1-D Brio-Wu, nx = 2^17, sigma = 1e4
         return synth.brio_wu_single(nx=2 ** 17, sigma=1e4)
     if name == "khi":               # the paper's Fig 8 workload: 512 x 1024 KHI, single fluid
         return synth.khi_paper(model=0)
     if name == "khi2f":             # ... two-fluid
         return synth.khi_paper(model=1)
-    if name == "tf3d":              # 3-D two-fluid blast, 128^3 (kernel studies; not a BASELINE config)
-        return synth.two_fluid_blast(n=128)
     raise SystemExit(f"unknown workload {name}")
 
 
@@ -564,9 +558,22 @@ def run_ours(args):
         cpu_base["sample_1thread"] = s1
     launches = sum(v["launches"] for v in kt.values())
     state_bytes = ((5 if nstage == 3 else 4) * NC + NH + 2 * NS) * ncell * 8
-    l2_note = ("state arrays (%.2f GB) exceed the 126 MB L2; no flush needed" % (state_bytes / 1e9) if state_bytes > 2 * 126e6 else
-               "state arrays (%.1f MB) fit in the 126 MB L2: this workload is timed L2-resident (launch-bound), as it runs in production; no flush"
-               % (state_bytes / 1e6))
+    # Three cases, not two: a working set between 1x and 4x the L2 is neither resident nor streamed from HBM every launch (each launch
+    # touches 1/3 to 1/2 of the state arrays, and the previous launch's output is still partly in L2 when the next one reads it)
+    L2_BYTES = 126e6
+    if state_bytes <= L2_BYTES:
+        l2_res = "fits"
+        l2_note = ("state arrays (%.1f MB) fit in the 126 MB L2: this workload is timed L2-resident (launch-bound), as it runs in "
+                   "production; no flush; the HBM fractions are L2-assisted" % (state_bytes / 1e6))
+    elif state_bytes <= 4 * L2_BYTES:
+        l2_res = "partly resident"
+        l2_note = ("state arrays (%.1f MB) are 1-4x the 126 MB L2: partly L2-resident from launch to launch, as it runs in production; "
+                   "no flush; the HBM fractions are L2-assisted" % (state_bytes / 1e6))
+    else:
+        l2_res = "exceeds"
+        l2_note = "state arrays (%.2f GB) exceed the 126 MB L2 several times; no flush needed" % (state_bytes / 1e9)
+    roof["l2_residency"] = l2_res
+    roof["l2_assisted"] = l2_res != "exceeds"      # true: hbm_frac / whole_step_hbm_frac count bytes that partly never left the L2
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,

@@ -90,7 +90,15 @@ int rmhd_set_cons(rmhd_ctx* c, const double* cons, const double* prim_guess, int
  * (reading G13): three implicit stages and three L evaluations, same kernels.  Everything runs on
  * the context's stream; one small device->host read of the statistics block (iteration histograms
  * and failure counters, about 1 KB) and a stream synchronisation at the end.
- * Returns NONCONVERGED if any root-find failed in any cell (the steps are still completed). */
+ * Returns NONCONVERGED if any root-find failed in any cell (the steps are still completed).
+ * Grids of at most 2^21 cells (every test-sized grid; cfg1, cfg3, cfg4 of BASELINE.json) are launch-bound: the first
+ * rmhd_step of such a context captures the launch sequence of one step on a private stream into a CUDA graph and every
+ * step replays it into the context's stream (same kernels, same arguments: bitwise the same state,
+ * tests/test_gpu_parity.py::test_graph_replay_equals_plain_launches_bitwise).  There is no switch for it; profiling mode
+ * (rmhd_set_profiling) uses plain launches so that each kernel can be timed; if capture fails the plain launches stay in force.
+ * rmhd_get_kernel_times counts a replayed step's kernels as launches like plain ones.  Consequences for the caller: do not
+ * call rmhd_step while p->stream is itself being captured, and do not drive one context from two host threads at once
+ * (a context, its graph and its statistics block are not guarded; use one context per thread). */
 int rmhd_step(rmhd_ctx* c, int nsteps);
 
 /* Copy out the interior state; either pointer may be NULL. */

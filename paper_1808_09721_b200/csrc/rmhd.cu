@@ -46,6 +46,8 @@ struct rmhd_ctx {
   cudaGraphExec_t step_graph;
   cudaStream_t cap_stream;
   bool graph_failed;
+  bool capturing;                    // build_step_graph is recording: launches are counted into graph_launches, not launches
+  long long graph_launches[5];       // launches of one captured step per kernel class, added to `launches` at every replay
   std::vector<EvRec> pending;
   std::vector<cudaEvent_t> ev_pool;
   double ms[KC_N];
@@ -101,7 +103,7 @@ cudaEvent_t get_event(rmhd_ctx* c) {
 struct Timed {
   rmhd_ctx* c; int cls; cudaEvent_t a, b;
   Timed(rmhd_ctx* c_, int cls_) : c(c_), cls(cls_), a(nullptr), b(nullptr) {
-    c->launches[cls]++;
+    if (c->capturing) c->graph_launches[cls]++; else c->launches[cls]++;
     if (c->profiling) { a = get_event(c); b = get_event(c); cudaEventRecord(a, c->stream); }
   }
   ~Timed() { if (c->profiling) { cudaEventRecord(b, c->stream); c->pending.push_back({cls, a, b}); } }
@@ -352,7 +354,10 @@ void build_step_graph(rmhd_ctx* c) {
   cudaGraph_t g = nullptr;
   if (cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeRelaxed) != cudaSuccess) { cudaGetLastError(); return; }
   c->stream = c->cap_stream;
+  c->capturing = true;
+  for (int i = 0; i < KC_N; ++i) c->graph_launches[i] = 0;
   const int rc = step_any(c);
+  c->capturing = false;
   c->stream = user;
   const cudaError_t e = cudaStreamEndCapture(c->cap_stream, &g);
   if (rc != RMHD_OK || e != cudaSuccess || !g) { if (g) cudaGraphDestroy(g); cudaGetLastError(); c->err.clear(); return; }
@@ -419,7 +424,8 @@ int rmhd_create(const rmhd_params* p, rmhd_ctx** out) {
   c->sm_count = 148;
   for (int i = 0; i < KC_N; ++i) { c->ms[i] = 0.0; c->launches[i] = 0; }
   c->q = c->w = c->qs = c->L1 = c->L2 = c->Ps1 = c->Ps2 = c->A = nullptr; c->d_stats = nullptr; c->h_stats = nullptr;
-  c->step_graph = nullptr; c->cap_stream = nullptr; c->graph_failed = false;
+  c->step_graph = nullptr; c->cap_stream = nullptr; c->graph_failed = false; c->capturing = false;
+  for (int i = 0; i < KC_N; ++i) c->graph_launches[i] = 0;
   DeviceGuard dg(c->device);
   { int n = 0; if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, c->device) == cudaSuccess && n > 0) c->sm_count = n; }
   const size_t rows = (size_t)((p->integrator == RMHD_SSP3_332 ? 5 : 4) * c->nc + c->nh + 2 * c->ns);
@@ -522,6 +528,7 @@ int rmhd_step(rmhd_ctx* c, int nsteps) {
     int rc;
     if (c->step_graph && !c->profiling) {
       CK(c, cudaGraphLaunch(c->step_graph, c->stream));
+      for (int i = 0; i < KC_N; ++i) c->launches[i] += c->graph_launches[i];
       rc = RMHD_OK;
     } else rc = step_any(c);
     if (rc) return rc;

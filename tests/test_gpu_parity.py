@@ -35,7 +35,13 @@ def rel_l1(a, b):
 
 
 PER_VAR_TOL = 1e-11            # resistive model (measured: <= 5e-13)
-PER_VAR_TOL_TWO_FLUID = 1e-13  # x mu^2: two-fluid model, 1e-9 for |mu| = 100 (measured: <= 1.5e-10), see rel_l1_per_var
+PER_VAR_TOL_TWO_FLUID = 1e-13  # x mu^2, capped at the case's global bound: two-fluid model, 1e-9 for |mu| = 100 (measured: <= 2.6e-10), see rel_l1_per_var
+
+
+def two_fluid_per_var_tol(mu, tol):
+    """1e-13 mu^2, but never looser than the global rel-L1 bound `tol` of the case: at |mu| >= 316 the mu^2 law would allow more
+    in one row than BASELINE.json allows in the sum over all rows (mu = 1e3: 1e-7 against 1e-8), and the check would say nothing."""
+    return min(PER_VAR_TOL_TWO_FLUID * mu ** 2, tol)
 
 
 def rel_l1_per_var(a, b, mu=None):
@@ -58,19 +64,23 @@ def rel_l1_per_var(a, b, mu=None):
     return np.array(out)
 
 
-def check_state(name, q, qo, tol, per_var_tol=None, mu=None):
-    """Global rel-L1 <= the BASELINE.json bound and every variable's rel-L1 <= 1e-11 (two-fluid: 1e-9); the measured values go to
+def check_state(name, q, qo, tol, params=None, per_var_tol=None):
+    """Global rel-L1 <= the BASELINE.json bound and every variable's rel-L1 <= 1e-11 (two-fluid: min(1e-13 mu^2, tol), mu = the larger
+    |mu_s| of the case's own `params`, which a two-fluid case must pass); the measured values go to
     gpurun_out/parity_values.jsonl when RMHD_PARITY_LOG is set (they are quoted in BASELINE.md section 4)."""
     two_fluid = qo.shape[0] == 18
-    if two_fluid and mu is None:
-        mu = 100.0
+    mu = None
+    if two_fluid:
+        assert params is not None and "mu_e" in params and "mu_p" in params, "two-fluid case: pass the case's params (mu_e, mu_p)"
+        mu = max(abs(params["mu_e"]), abs(params["mu_p"]))
     if per_var_tol is None:
-        per_var_tol = PER_VAR_TOL_TWO_FLUID * mu ** 2 if two_fluid else PER_VAR_TOL
-    g = float(rel_l1(q, qo)); pv = rel_l1_per_var(q, qo, mu if two_fluid else None)
+        per_var_tol = two_fluid_per_var_tol(mu, tol) if two_fluid else PER_VAR_TOL
+    g = float(rel_l1(q, qo)); pv = rel_l1_per_var(q, qo, mu)
     if os.environ.get("RMHD_PARITY_LOG"):
         os.makedirs("gpurun_out", exist_ok=True)
         with open("gpurun_out/parity_values.jsonl", "a") as f:
-            f.write(json.dumps({"case": name, "rel_l1": g, "per_var_max": float(pv.max()), "per_var": [float(x) for x in pv]}) + "\n")
+            f.write(json.dumps({"case": name, "rel_l1": g, "per_var_max": float(pv.max()), "per_var_tol": per_var_tol,
+                                "per_var": [float(x) for x in pv]}) + "\n")
     assert g <= tol, (name, g)
     assert pv.max() <= per_var_tol, (name, int(pv.argmax()), pv)
     return g, pv
@@ -281,7 +291,7 @@ def _random_state(model, shape, seed):
     (0, (1, 1, 67), (0, 0, 0)), (0, (1, 1, 130), (1, 1, 1)), (0, (1, 9, 70), (1, 0, 0)), (0, (1, 33, 5), (0, 1, 0)),
     (0, (7, 10, 35), (0, 1, 0)), (0, (11, 3, 66), (1, 0, 1)), (0, (9, 1, 40), (0, 0, 1)),
     (0, (37, 6, 33), (1, 1, 1)), (0, (50, 5, 40), (0, 0, 0)), (0, (2, 2, 2), (1, 0, 1)), (1, (35, 6, 33), (0, 1, 1)),
-    # even nx, 3-D, resistive: the TMA-staged kernel (flux_vp.cuh); partial tiles in x and y, several z segments, both BCs
+    # even nx, 3-D, resistive: partial x / y tiles and several z segments of k_flux_hm with 8-row tiles (ny >= 8) and 4-row tiles, both BCs
     (0, (7, 10, 34), (0, 1, 0)), (0, (20, 19, 70), (1, 0, 1)), (0, (5, 8, 32), (0, 0, 0)), (0, (40, 16, 64), (1, 1, 1)),
     (0, (3, 2, 4), (1, 1, 0)), (0, (33, 9, 30), (0, 0, 1)),
     (1, (1, 1, 67), (1, 0, 0)), (1, (1, 12, 37), (0, 1, 0)), (1, (6, 9, 34), (1, 1, 0)),
@@ -319,7 +329,7 @@ def test_config1_riemann_tube_full(B, O, synth):
     q, w, st = run_gpu(B, c)
     qo, wo, sto = run_oracle(O, c)
     assert st["n_failed"] == 0
-    check_state("cfg1 128 cells x 128 steps", q, qo, 1e-9)
+    check_state("cfg1 128 cells x 128 steps", q, qo, 1e-9, c["params"])
     assert st["hist_stage"].sum() == 2 * 128 * 128 and st["hist_c2p"].sum() == 128 * 128
     assert st["hist_stage"][0] == 0
 
@@ -329,7 +339,7 @@ def test_config3_shear_layer_reduced(B, O, synth):
     q, w, st = run_gpu(B, c)
     qo, wo, _ = run_oracle(O, c)
     assert st["n_failed"] == 0
-    check_state("cfg3 96 x 128 x 60 steps", q, qo, 1e-8)
+    check_state("cfg3 96 x 128 x 60 steps", q, qo, 1e-8, c["params"])
     assert rel_l1(w[:5], wo[:5]) <= 1e-8
 
 
@@ -341,7 +351,7 @@ def test_config3_shear_layer_full_size(B, O, synth):
     q, w, st = run_gpu(B, c)
     qo, wo, _ = run_oracle(O, c)
     assert st["n_failed"] == 0
-    check_state("cfg3 512 x 512 x 200 steps", q, qo, 1e-8)
+    check_state("cfg3 512 x 512 x 200 steps", q, qo, 1e-8, c["params"])
     assert rel_l1(w[:5], wo[:5]) <= 1e-8
 
 
@@ -350,15 +360,15 @@ def test_config5_blast_reduced(B, O, synth):
     q, w, st = run_gpu(B, c)
     qo, wo, _ = run_oracle(O, c)
     assert st["n_failed"] == 0
-    check_state("cfg5 40^3 x 20 steps", q, qo, 1e-8)
+    check_state("cfg5 40^3 x 20 steps", q, qo, 1e-8, c["params"])
 
 
 def test_config5_full_size_full_length(B, O, synth):
     """BASELINE.json configs[4] as stated: 256^3, 20 steps, the WHOLE grid against the oracle, in the launch configuration
     bench.py times.  Cost: 256^3 x 20 = 3.4e8 oracle zone-updates, about 6 minutes at the 9e5 zone-updates/s the oracle
     reaches on the GPU box's 16 host threads, and about 25 GB of host memory (the oracle keeps 120 ghosted rows of
-    264^3 doubles).  RMHD_CFG5_FULL_N overrides the edge length (a smaller box for a quick look)."""
-    n = int(os.environ.get("RMHD_CFG5_FULL_N", "256"))
+    264^3 doubles)."""
+    n = 256
     c = synth.config5(n=n, nsteps=20)
     assert c["nsteps"] == 20
     t0 = time.time()
@@ -367,7 +377,7 @@ def test_config5_full_size_full_length(B, O, synth):
     qo, wo, sto = run_oracle(O, c)
     del wo
     assert st["n_failed"] == 0 and sto["n_failed"] == 0
-    g, pv = check_state("cfg5 %d^3 x 20 steps (whole grid)" % n, q, qo, 1e-8)
+    g, pv = check_state("cfg5 %d^3 x 20 steps (whole grid)" % n, q, qo, 1e-8, c["params"])
     assert st["hist_stage"].sum() == 2 * n ** 3 * 20
     print("cfg5 full: %.0f s, rel-L1 %.2e, per-variable max %.2e" % (time.time() - t0, g, pv.max()))
 
@@ -413,7 +423,7 @@ def test_config4_two_fluid_reduced(B, O, synth):
     q, w, st = run_gpu(B, c)
     qo, wo, _ = run_oracle(O, c)
     assert st["n_failed"] == 0
-    check_state("cfg4 64 x 48 x 50 steps", q, qo, 1e-8)
+    check_state("cfg4 64 x 48 x 50 steps", q, qo, 1e-8, c["params"])
     assert rel_l1(w[:10], wo[:10]) <= 1e-8
     assert st["hist_stage"].sum() == 2 * 64 * 48 * 50
 
@@ -427,7 +437,7 @@ def test_config4_full_size_full_length(B, O, synth):
     q, w, st = run_gpu(B, c)
     qo, wo, sto = run_oracle(O, c)
     assert st["n_failed"] == 0 and sto["n_failed"] == 0
-    g, pv = check_state("cfg4 1024 x 1024 x 50 steps (whole grid)", q, qo, 1e-8)
+    g, pv = check_state("cfg4 1024 x 1024 x 50 steps (whole grid)", q, qo, 1e-8, c["params"])
     assert rel_l1(w[:10], wo[:10]) <= 1e-8
     assert st["hist_stage"].sum() == 2 * 1024 * 1024 * 50
     print("cfg4 full: %.0f s, rel-L1 %.2e, per-variable max %.2e" % (time.time() - t0, g, pv.max()))
@@ -475,17 +485,22 @@ def test_unphysical_input_is_reported(B, synth):
 
 def test_graph_replay_equals_plain_launches_bitwise(B, synth):
     """rmhd_step replays one captured step as a CUDA graph on grids of up to 2^21 cells; profiling mode uses plain launches.
-    Same kernels, same arguments: the states must be bitwise equal (1-D, 2-D and 3-D, both integrators)."""
+    Same kernels, same arguments: the states must be bitwise equal (1-D, 2-D and 3-D, both integrators), and
+    rmhd_get_kernel_times must count the same launches on both paths (a replayed step counts its kernels, the capture itself none)."""
     for c, kw in ((synth.config1(nx=100), {}), (synth.config3(nx=64, ny=40, nsteps=6), {}), (synth.config5(n=24, nsteps=6), {}),
                   (synth.config5(n=24, nsteps=6), {"integrator": "ssp3"}), (synth.config4(nx=40, ny=24, nsteps=6), {})):
         p = dict(c["params"]); p.update(kw)
         a = B.Rmhd(**p); a.set_initial(np.ascontiguousarray(c["prims"]), c.get("rho_charge"))
+        B.rmhd_set_profiling(a.ctx, False)      # zeroes the counters; set_initial's launch is not a step's
         a.step(1); a.step(5)
+        la = {k: v["launches"] for k, v in B.rmhd_get_kernel_times(a.ctx).items()}
         qa, wa = a.get_state(); sa = a.stats(); a.close()
         b = B.Rmhd(**p); b.set_initial(np.ascontiguousarray(c["prims"]), c.get("rho_charge"))
         B.rmhd_set_profiling(b.ctx, True)
         b.step(6)
+        lb = {k: v["launches"] for k, v in B.rmhd_get_kernel_times(b.ctx).items()}
         qb, wb = b.get_state(); sb = b.stats(); b.close()
+        assert la == lb and sum(la.values()) == 6 * (7 if kw else 5), (la, lb)
         assert np.array_equal(qa, qb) and np.array_equal(wa, wb)
         assert np.array_equal(sa["hist_stage"], sb["hist_stage"]) and np.array_equal(sa["hist_c2p"], sb["hist_c2p"])
 
@@ -547,7 +562,7 @@ def test_ssp3_332_parity(B, O, synth, case, monkeypatch):
     q, w, st = run_gpu(B, c, nsteps=nsteps, params_override={"integrator": "ssp3"})
     qo, wo, _ = run_oracle(O, c, nsteps=nsteps, params_override={"integrator": "ssp3"})
     assert st["n_failed"] == 0
-    check_state("ssp3 " + case, q, qo, tol)
+    check_state("ssp3 " + case, q, qo, tol, c["params"])
     ncell = int(np.prod(c["prims"].shape[1:]))
     assert st["hist_stage"].sum() == 3 * ncell * nsteps and st["hist_c2p"].sum() == ncell * nsteps
     # and it is a different scheme from SSP2(222)
@@ -579,7 +594,7 @@ def test_paper_setups_parity(B, O, synth, case, integrator):
     q, w, st = run_gpu(B, c)
     qo, wo, sto = run_oracle(O, c)
     assert st["n_failed"] == 0 and sto["n_failed"] == 0
-    check_state("paper %s %s" % (case, integrator), q, qo, tol, mu=max(abs(c["params"].get("mu_e", 0.0)), abs(c["params"].get("mu_p", 0.0))))
+    check_state("paper %s %s" % (case, integrator), q, qo, tol, c["params"])
     nh = 5 if c["params"]["model"] == 0 else 10
     assert rel_l1(w[:nh], wo[:nh]) <= 10 * tol
 
@@ -593,7 +608,7 @@ def test_two_fluid_3d_blast_parity(B, O, synth, integrator, flux, monkeypatch):
     q, w, st = run_gpu(B, c)
     qo, wo, sto = run_oracle(O, c)
     assert st["n_failed"] == 0 and sto["n_failed"] == 0
-    check_state("two-fluid 3-D blast %s %s" % (integrator, flux), q, qo, 1e-8)
+    check_state("two-fluid 3-D blast %s %s" % (integrator, flux), q, qo, 1e-8, c["params"])
     assert rel_l1(w[:10], wo[:10]) <= 1e-8
 
 
