@@ -438,8 +438,10 @@ def run_ours(args):
         barrier()
     ms_total = ev0.elapsed_time(ev1)
     B.rmhd_set_profiling(sim.ctx, True)
+    B.rmhd_debug_hm_cycles(local, reset=True)           # None unless this is a measurement build (-DRMHD_HM_CYCLES)
     sim.step(args.steps)
     kt = B.rmhd_get_kernel_times(sim.ctx)
+    hm_cycles = B.rmhd_debug_hm_cycles(local)
     stats = sim.stats()
     B.rmhd_set_profiling(sim.ctx, False)
     value, ms_total = whole_job_rate(ms_total, ncell * args.steps, dist, dev)
@@ -503,6 +505,11 @@ def run_ours(args):
     roof["avg_launch_ms"] = avg_ms
     roof["kernel_time_shares"] = shares
     roof["kernel_ms_per_step"] = {k: v["ms"] / args.steps for k, v in kt.items()}
+    if hm_cycles is not None:   # measurement build: clock() ticks per warp and plane, by role and phase (csrc/flux_hm.cuh); never a bench number
+        roof["hm_cycles_per_warp_plane"] = {r: [float(hm_cycles[i][ph]) / max(float(hm_cycles[i][7]), 1.0) for ph in range(7)]
+                                            for i, r in enumerate(("H", "M"))}
+        roof["hm_warp_planes"] = [int(hm_cycles[0][7]), int(hm_cycles[1][7])]
+        roof["measurement_build"] = "-DRMHD_HM_CYCLES: the times of this line are perturbed by the instrumentation"
     # DRAM bytes per launch from the committed ncu capture of exactly these kernel sources, else null
     cap = committed_ncu(args.workload, args.integrator)
     roof["traffic"] = None

@@ -283,6 +283,18 @@ def rmhd_flux_divergence_static(params, cons, Lout, check=True):
     return rc, nf.value
 
 
+def rmhd_debug_hm_cycles(device=0, reset=False):
+    """Cycle account of k_flux_hm ([role H | M][phase 0..6, warp-planes], csrc/flux_hm.cuh), or None: only a measurement build
+    of the library (-DRMHD_HM_CYCLES) exports it."""
+    L = lib()
+    if not hasattr(L, "rmhd_debug_hm_cycles"):
+        return None
+    out = np.zeros((2, 8), dtype=np.uint64)
+    L.rmhd_debug_hm_cycles.argtypes = [C.c_int, C.c_void_p, C.c_int]
+    _check(L.rmhd_debug_hm_cycles(device, out.ctypes.data, int(bool(reset))))
+    return out
+
+
 def rmhd_probe_fp64(device=0, stream=None):
     v = C.c_double(0.0)
     _check(lib().rmhd_probe_fp64(device, _current_stream(device) if stream is None else stream, C.byref(v)))

@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
-LIB = os.path.join(HERE, "librmhd.so")
+LIB = os.environ.get("RMHD_LIB") or os.path.join(HERE, "librmhd.so")   # RMHD_LIB: build (and, binding.py, load) another copy, e.g. a measurement build
 SOURCES = [os.path.join(CSRC, "rmhd.cu")]
 HEADERS = [os.path.join(CSRC, f) for f in ("physics.cuh", "stage.cuh", "kernels.cuh", "flux_fused.cuh", "flux_hm.cuh")] + [os.path.join(ROOT, "include", "rmhd.h")]
 

@@ -86,6 +86,36 @@ template <int MODEL> __host__ __device__ constexpr int hm_mrow(int m) {   // con
 #define RMHD_HM_GH 6     // reconstructions in flight per batch, role H (12 per face)
 #endif
 
+// Cycle account of the plane loop (measurement build only: -DRMHD_HM_CYCLES; the product library has none of it).  Lane 0 of
+// every warp adds the clock() ticks between two marks to a global counter [role][phase]; the marks sit where the phases of
+// the plane loop end.  Phases, role H: 0 own-cell loads + flux vectors + field stores, 1 bar.sync, 2 x/y reconstructions,
+// 3 z part, 4 mbarrier wait, 5 epilogue (fY / fX reads, stores), 6 z part of the feed-only prologue planes.  Role M: 0 z part
+// + own-cell field stores, 1 halo cells, 2 bar.sync, 3 x/y reconstructions + extra faces, 4 mbarrier arrive + wait, 5 epilogue,
+// 6 prologue planes.  Slot 7 counts the warp-planes.  Loads are charged where their consumer waits, not where they issue.
+#ifdef RMHD_HM_CYCLES
+__device__ unsigned long long g_hm_cycles[2][8];
+#define HM_TICK_DECL() __shared__ unsigned hm_acc[32][8]; if (threadIdx.x < 256) hm_acc[threadIdx.x >> 3][threadIdx.x & 7] = 0u
+#define HM_TICK_START() unsigned hm_t0 = (unsigned)clock()
+#define HM_TICK(ph)                                                      \
+  do {                                                                   \
+    const unsigned hm_t1 = (unsigned)clock();                            \
+    if (lane == 0) hm_acc[wrp][(ph)] += hm_t1 - hm_t0;                   \
+    hm_t0 = hm_t1;                                                       \
+  } while (0)
+#define HM_COUNT_PLANE() do { if (lane == 0) hm_acc[wrp][7] += 1u; } while (0)
+#define HM_TICK_FLUSH()                                                                                           \
+  do {                                                                                                            \
+    if (lane == 0)                                                                                                \
+      for (int ph = 0; ph < 8; ++ph) atomicAdd(&g_hm_cycles[roleH ? 0 : 1][ph], (unsigned long long)hm_acc[wrp][ph]); \
+  } while (0)
+#else
+#define HM_TICK_START() do {} while (0)
+#define HM_TICK(ph) do {} while (0)
+#define HM_COUNT_PLANE() do {} while (0)
+#define HM_TICK_DECL() do {} while (0)
+#define HM_TICK_FLUSH() do {} while (0)
+#endif
+
 // HAS_Y = false (2-D grids): the tile's TY rows are TY consecutive 32-cell segments of one x line, there is no y work in
 // the plane, and the marching axis ("z" below) is the grid's y axis: ZDIR = 1 selects the y components of the flux
 // vectors; the host passes ny = 1, nz = the grid's ny, bcz = its y boundary condition, hidz = 1/(2 dy).  A 2-D grid
@@ -106,6 +136,7 @@ k_flux_hm(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, size_
   extern __shared__ double sm[];
   __shared__ unsigned long long bar2;                // "P2 done" (fY, fX written; gX, gY no longer read)
   if (threadIdx.x == 0) mbar_init(&bar2, NT);
+  HM_TICK_DECL();
   __syncthreads();
   unsigned ph2 = 0;
   double* gX = sm;
@@ -167,6 +198,8 @@ k_flux_hm(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, size_
     double Lacc[NR];                                 // H: 6 rows (D, S, tau, rho_charge); M: 8 rows (B, E, psi, phi)
 #pragma unroll
     for (int v = 0; v < NR; ++v) Lacc[v] = 0.0;
+    HM_TICK_START();
+    if (do_xy) HM_COUNT_PLANE();
 
     if (roleH) {
       // ======================================= role H =======================================
@@ -193,7 +226,9 @@ k_flux_hm(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, size_
             }
           }
         }
+        HM_TICK(0);
         hm_barrier<NT>();
+        HM_TICK(1);
         // left x-face (t = 0) and bottom y-face (t = 1) of the own cell: ONE copy of the reconstruction code
 #pragma unroll 1
         for (int t = 0; t < (HAS_Y ? 2 : 1); ++t) {
@@ -216,6 +251,7 @@ k_flux_hm(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, size_
           }
         }
         mbar_arrive(&bar2);                          // waited for after the z part
+        HM_TICK(2);
       }
       if (HAS_Z) {
         double u0[2 * NHV];
@@ -254,9 +290,11 @@ k_flux_hm(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, size_
 #pragma unroll
         for (int f = 0; f < 2 * NHV; ++f) ring[s_old + f * MAIN] = u0[f];
         { const int t = s_old; s_old = s_new; s_new = t; }
+        HM_TICK(do_xy ? 3 : 6);
       }
       if (do_xy) {
         mbar_wait(&bar2, ph2); ph2 ^= 1u;
+        HM_TICK(4);
 #pragma unroll
         for (int h = 0; h < NHV; ++h) if (HAS_Y) Lacc[h] = fma(-fY[(FS::hv(h) * (TY + 1) + ty + 1) * TX + lane], hidy, Lacc[h]);
         if (lane == 31) {
@@ -267,6 +305,7 @@ k_flux_hm(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, size_
           const unsigned id = pk + (unsigned)j * nx + i;
           store_rows<COMB, NHV, MODEL>(L, cb, N, id, Lacc, [](int h) { return FS::hv(h); });
         }
+        HM_TICK(5);
       }
     } else {
       // ======================================= role M =======================================
@@ -316,6 +355,7 @@ k_flux_hm(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, size_
           for (int v = 0; v < NM; ++v) { if (do_xy) Lacc[v] = (Gprev[v] - G[v]) * hidz; Gprev[v] = G[v]; }
         }
       }
+      HM_TICK(do_xy ? 0 : 6);
       if (do_xy) {
         {
           double q_[NC], w_[NH], g[NF];
@@ -335,7 +375,9 @@ k_flux_hm(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, size_
             for (int f = 0; f < NF; ++f) gX[(f * TY + xh_row) * XW + xh_col] = g[f];
           }
         }
+        HM_TICK(1);
         hm_barrier<NT>();
+        HM_TICK(2);
         // t = 0: left x-face, t = 1: bottom y-face of the own cell; t = 2 (two M warps only): the last row of
         // y-faces / the 33rd x-face of row `lane` (lanes >= TY reconstruct in-bounds garbage that is not stored)
         constexpr int XB = TY == 4 ? 0 : 4;          // first of the 4 M warps that take the extra faces (TY = 8: those without a y-halo row)
@@ -377,8 +419,10 @@ k_flux_hm(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, size_
             for (int h = 0; h < NHV; ++h) fX[FS::hv(h) * TY + lane] = o[h] + o[NHV + h];
           }
         }
+        HM_TICK(3);
         mbar_arrive(&bar2);
         mbar_wait(&bar2, ph2); ph2 ^= 1u;
+        HM_TICK(4);
 #pragma unroll
         for (int v = 0; v < NM; ++v) if (HAS_Y) Lacc[v] = fma(-fY[(hm_mrow<MODEL>(v) * (TY + 1) + ty + 1) * TX + lane], hidy, Lacc[v]);
         if (lane == 31) {
@@ -389,9 +433,11 @@ k_flux_hm(ConsRows<MODEL> qin, HydRows<MODEL> win, double* __restrict__ L, size_
           const unsigned id = pk + (unsigned)j * nx + i;
           store_rows<COMB, NM, MODEL>(L, cb, N, id, Lacc, [](int m) { return hm_mrow<MODEL>(m); });
         }
+        HM_TICK(5);
       }
     }
   }
+  HM_TICK_FLUSH();
 }
 
 }  // namespace rmhd

@@ -886,3 +886,17 @@ extern "C" int rmhd_flux_divergence_static(const rmhd_params* p, const double* c
   if (h.n_failed) { g_create_error = "rmhd_flux_divergence_static: primitive recovery failed in some cells (count in *n_failed); L is not valid near them"; return RMHD_ERR_NONCONVERGED; }
   return RMHD_OK;
 }
+
+// ---- measurement build only (-DRMHD_HM_CYCLES, flux_hm.cuh): read / clear the cycle account of k_flux_hm ---------------
+#ifdef RMHD_HM_CYCLES
+extern "C" int rmhd_debug_hm_cycles(int device, unsigned long long* out16, int reset) {
+  DeviceGuard dg(device);
+  if (cudaDeviceSynchronize() != cudaSuccess) return RMHD_ERR_CUDA;
+  if (out16 && cudaMemcpyFromSymbol(out16, g_hm_cycles, sizeof(unsigned long long) * 16) != cudaSuccess) return RMHD_ERR_CUDA;
+  if (reset) {
+    unsigned long long z[16] = {};
+    if (cudaMemcpyToSymbol(g_hm_cycles, z, sizeof z) != cudaSuccess) return RMHD_ERR_CUDA;
+  }
+  return RMHD_OK;
+}
+#endif
