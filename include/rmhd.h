@@ -131,7 +131,17 @@ void rmhd_destroy(rmhd_ctx* c);
 /* ---- batched per-cell operations on n independent cells (BASELINE.json configs[1]) --------- */
 /* Only model, gamma, sigma, eta, mu_e, mu_p, kappa, tolerances, device and stream of *p are
  * used.  All pointers are DEVICE pointers unless on_device == 0, in which case the call
- * stages them through temporary device buffers (host<->device copies inside the call). */
+ * stages them through the library's staging area on p->device (host<->device copies inside the call; see
+ * rmhd_release_staging below).  With on_device == 1 the calls only launch a kernel on p->stream and return. */
+
+/* Staging memory of the on_device == 0 calls: one grow-only device allocation per GPU, made by the first such call,
+ * enlarged when a later call needs more, and kept between calls, so that a loop over host batches does not pay a
+ * cudaMalloc / cudaFree pair per buffer and call (cudaFree synchronises the whole device).  Host-buffer batch calls of one
+ * process run one at a time (the staging area is locked for the duration of a call).  rmhd_release_staging frees it:
+ * device >= 0 that GPU's, device < 0 every GPU's; it is an error to call it while a host-buffer batch call is running on
+ * another thread only in the sense that it waits for that call.  Nothing else in the library keeps memory after rmhd_destroy
+ * (except the fixed array of rmhd_flux_divergence_static, which is part of the library image). */
+int rmhd_release_staging(int device);
 
 /* One implicit stage (eq 10):  q* - q_ex - a_dt Psi(q*) = 0 per cell.
  * (SURVEY.md 8(b) lists `model` and `stream` as arguments: both travel in *p here.)

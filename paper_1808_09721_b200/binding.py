@@ -28,7 +28,7 @@ EXPORTS = (
     "rmhd_create", "rmhd_set_initial", "rmhd_set_cons", "rmhd_step", "rmhd_get_state", "rmhd_flux_divergence",
     "rmhd_get_stats", "rmhd_set_profiling", "rmhd_get_kernel_times", "rmhd_dt", "rmhd_time", "rmhd_last_error",
     "rmhd_destroy", "rmhd_stage_batch", "rmhd_prim2cons_batch", "rmhd_con2prim_batch", "rmhd_probe_fp64",
-    "rmhd_probe_hbm", "rmhd_flux_divergence_static",
+    "rmhd_probe_hbm", "rmhd_flux_divergence_static", "rmhd_release_staging",
 )
 RMHD_STATIC_MAX_CELLS = 262144   # include/rmhd.h: capacity of the library's fixed scratch array (rmhd_flux_divergence_static)
 
@@ -118,6 +118,7 @@ def lib():
     L.rmhd_probe_fp64.argtypes = [C.c_int, vp, _dp]
     L.rmhd_probe_hbm.argtypes = [C.c_int, vp, C.c_longlong, _dp]
     L.rmhd_flux_divergence_static.argtypes = [pp, vp, vp, _lp]
+    L.rmhd_release_staging.argtypes = [C.c_int]
     _lib = L
     return L
 
@@ -281,6 +282,11 @@ def rmhd_flux_divergence_static(params, cons, Lout, check=True):
     if check:
         _check(rc)
     return rc, nf.value
+
+
+def rmhd_release_staging(device=-1):
+    """Free the staging area the host-buffer batch calls keep on `device` (-1: on every GPU)."""
+    _check(lib().rmhd_release_staging(int(device)))
 
 
 def rmhd_debug_hm_cycles(device=0, reset=False):

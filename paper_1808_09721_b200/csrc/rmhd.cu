@@ -612,21 +612,41 @@ int rmhd_get_kernel_times(rmhd_ctx* c, double* ms, long long* launches, int n) {
 
 // ---- batched per-cell operations -----------------------------------------------------------
 namespace {
-struct Staging {   // device copies of host buffers for the on_device == 0 path
+// Device copies of host buffers for the on_device == 0 path.  They are carved out of ONE grow-only allocation per device that
+// outlives the call (rmhd_release_staging frees it): a caller who feeds host batches in a loop pays cudaMalloc once, not
+// up to seven cudaMalloc + cudaFree per call (each cudaFree synchronises the device).  The arena's mutex is held for the whole
+// call: host-buffer batch calls on one process serialise, which they did in effect before (every one ends in a stream synchronise).
+constexpr int STAGING_MAX_DEVICES = 64;
+struct StagingArena { void* base; size_t cap; };
+StagingArena g_staging[STAGING_MAX_DEVICES];
+std::mutex g_staging_mu;
+inline size_t staging_align(size_t b) { return (b + 255) & ~(size_t)255; }
+struct Staging {
   cudaStream_t s;
-  std::vector<void*> bufs;
-  explicit Staging(cudaStream_t s_) : s(s_) {}
-  ~Staging() { for (void* b : bufs) cudaFree(b); }
-  template <class T> cudaError_t in(const T* host, size_t n, const T** dev) {
-    if (!host) { *dev = nullptr; return cudaSuccess; }
-    void* d = nullptr; cudaError_t e = cudaMalloc(&d, sizeof(T) * n); if (e != cudaSuccess) return e;
-    bufs.push_back(d); *dev = (const T*)d;
+  int dev;
+  size_t used;
+  std::unique_lock<std::mutex> lk;
+  Staging(cudaStream_t s_, int dev_) : s(s_), dev(dev_), used(0), lk(g_staging_mu) {}
+  // make room for `bytes` (the sum of staging_align(size) over the buffers of this call); the device must be current
+  cudaError_t reserve(size_t bytes) {
+    if (dev < 0 || dev >= STAGING_MAX_DEVICES) return cudaErrorInvalidDevice;
+    StagingArena& a = g_staging[dev];
+    if (a.cap >= bytes) return cudaSuccess;
+    if (a.base) { cudaFree(a.base); a.base = nullptr; a.cap = 0; }
+    const size_t want = (bytes + ((size_t)1 << 20) - 1) & ~(((size_t)1 << 20) - 1);
+    const cudaError_t e = cudaMalloc(&a.base, want);
+    if (e == cudaSuccess) a.cap = want; else a.base = nullptr;
+    return e;
+  }
+  void* take(size_t bytes) { void* d = (char*)g_staging[dev].base + used; used += staging_align(bytes); return d; }
+  template <class T> cudaError_t in(const T* host, size_t n, const T** dev_ptr) {
+    if (!host) { *dev_ptr = nullptr; return cudaSuccess; }
+    void* d = take(sizeof(T) * n); *dev_ptr = (const T*)d;
     return cudaMemcpyAsync(d, host, sizeof(T) * n, cudaMemcpyHostToDevice, s);
   }
-  template <class T> cudaError_t out(T* host, size_t n, T** dev) {
-    if (!host) { *dev = nullptr; return cudaSuccess; }
-    void* d = nullptr; cudaError_t e = cudaMalloc(&d, sizeof(T) * n); if (e != cudaSuccess) return e;
-    bufs.push_back(d); *dev = (T*)d;
+  template <class T> cudaError_t out(T* host, size_t n, T** dev_ptr) {
+    if (!host) { *dev_ptr = nullptr; return cudaSuccess; }
+    *dev_ptr = (T*)take(sizeof(T) * n);
     return cudaSuccess;
   }
 };
@@ -657,10 +677,19 @@ int rmhd_stage_batch(const rmhd_params* p, long long ncells, const double* q_ex,
   cudaStream_t s = (cudaStream_t)p->stream;
   const size_t N = (size_t)ncells;
   const int nc = p->model == 0 ? 14 : 18, np = p->model == 0 ? 11 : 16;
-  Staging st(s);
   const double *d_qex = q_ex, *d_pg = prim_guess, *d_sig = sigma_cell;
   double *d_qo = q_out, *d_po = prims_out; int *d_it = iters, *d_fl = fail;
-  if (!on_device) {
+  if (on_device) {
+    if (p->model == 0) k_stage_batch_resistive<<<blocks_for(N, 128), 128, 0, s>>>(d_qex, d_pg, d_sig, a_dt, d_qo, d_po, d_it, d_fl, N, P);
+    else k_stage_batch_two_fluid<<<blocks_for(N, 128), 128, 0, s>>>(d_qex, d_pg, a_dt, d_qo, d_po, d_it, d_fl, N, P);
+    CK(nullptr, cudaGetLastError());
+    return RMHD_OK;
+  }
+  Staging st(s, p->device);
+  {
+    const size_t D = sizeof(double), I = sizeof(int);
+    CK(nullptr, st.reserve(2 * staging_align(D * nc * N) + 2 * staging_align(D * np * N) + (sigma_cell ? staging_align(D * N) : 0) +
+                           (iters ? staging_align(I * N) : 0) + (fail ? staging_align(I * N) : 0)));
     CK(nullptr, st.in(q_ex, nc * N, &d_qex)); CK(nullptr, st.in(prim_guess, np * N, &d_pg)); CK(nullptr, st.in(sigma_cell, N, &d_sig));
     CK(nullptr, st.out(q_out, nc * N, &d_qo)); CK(nullptr, st.out(prims_out, np * N, &d_po));
     CK(nullptr, st.out(iters, N, &d_it)); CK(nullptr, st.out(fail, N, &d_fl));
@@ -689,8 +718,15 @@ int rmhd_prim2cons_batch(const rmhd_params* p, long long ncells, const double* p
   cudaStream_t s = (cudaStream_t)p->stream;
   const size_t N = (size_t)ncells;
   const int nc = p->model == 0 ? 14 : 18, np = p->model == 0 ? 11 : 16;
-  Staging st(s);
   const double *d_pr = prims, *d_rc = rho_charge; double* d_co = cons;
+  if (on_device) {
+    if (p->model == 0) k_prim2cons_batch<0><<<blocks_for(N, 256), 256, 0, s>>>(d_pr, d_rc, d_co, N, P);
+    else k_prim2cons_batch<1><<<blocks_for(N, 256), 256, 0, s>>>(d_pr, nullptr, d_co, N, P);
+    CK(nullptr, cudaGetLastError());
+    return RMHD_OK;
+  }
+  Staging st(s, p->device);
+  CK(nullptr, st.reserve(staging_align(sizeof(double) * np * N) + (rho_charge ? staging_align(sizeof(double) * N) : 0) + staging_align(sizeof(double) * nc * N)));
   if (!on_device) { CK(nullptr, st.in(prims, np * N, &d_pr)); CK(nullptr, st.in(rho_charge, N, &d_rc)); CK(nullptr, st.out(cons, nc * N, &d_co)); }
   if (p->model == 0) k_prim2cons_batch<0><<<blocks_for(N, 256), 256, 0, s>>>(d_pr, d_rc, d_co, N, P);
   else k_prim2cons_batch<1><<<blocks_for(N, 256), 256, 0, s>>>(d_pr, nullptr, d_co, N, P);
@@ -710,9 +746,18 @@ int rmhd_con2prim_batch(const rmhd_params* p, long long ncells, const double* co
   cudaStream_t s = (cudaStream_t)p->stream;
   const size_t N = (size_t)ncells;
   const int nc = p->model == 0 ? 14 : 18, np = p->model == 0 ? 11 : 16, nh = p->model == 0 ? 5 : 10;
-  Staging st(s);
   const double *d_co = cons, *d_pg = prim_guess; double* d_pr = prims; int *d_it = iters, *d_fl = fail;
-  if (!on_device) {
+  if (on_device) {
+    if (p->model == 0) k_con2prim<0><<<blocks_for(N, 256), 256, 0, s>>>(d_co, d_pg, N, d_pr, N, d_pr + (size_t)nh * N, d_it, d_fl, N, P, nullptr);
+    else k_con2prim<1><<<blocks_for(N, 256), 256, 0, s>>>(d_co, d_pg, N, d_pr, N, d_pr + (size_t)nh * N, d_it, d_fl, N, P, nullptr);
+    CK(nullptr, cudaGetLastError());
+    return RMHD_OK;
+  }
+  Staging st(s, p->device);
+  {
+    const size_t D = sizeof(double), I = sizeof(int);
+    CK(nullptr, st.reserve(staging_align(D * nc * N) + (prim_guess ? staging_align(D * np * N) : 0) + staging_align(D * np * N) +
+                           (iters ? staging_align(I * N) : 0) + (fail ? staging_align(I * N) : 0)));
     CK(nullptr, st.in(cons, nc * N, &d_co)); CK(nullptr, st.in(prim_guess, np * N, &d_pg)); CK(nullptr, st.out(prims, np * N, &d_pr));
     CK(nullptr, st.out(iters, N, &d_it)); CK(nullptr, st.out(fail, N, &d_fl));
   }
@@ -726,6 +771,18 @@ int rmhd_con2prim_batch(const rmhd_params* p, long long ncells, const double* co
     CK(nullptr, cudaStreamSynchronize(s));
   }
   return RMHD_OK;
+}
+
+int rmhd_release_staging(int device) {
+  std::lock_guard<std::mutex> lk(g_staging_mu);
+  int rc = RMHD_OK;
+  for (int d = 0; d < STAGING_MAX_DEVICES; ++d) {
+    if ((device >= 0 && d != device) || !g_staging[d].base) continue;
+    DeviceGuard dg(d);
+    if (cudaFree(g_staging[d].base) != cudaSuccess) { cudaGetLastError(); rc = RMHD_ERR_CUDA; }
+    g_staging[d].base = nullptr; g_staging[d].cap = 0;
+  }
+  return rc;
 }
 
 // ---- probes ----------------------------------------------------------------------------------

@@ -114,3 +114,9 @@ def test_the_one_environment_switch_is_documented(B):
     assert envs == {"RMHD_FLUX"}
     hdr = open(os.path.join(ROOT, "include", "rmhd.h")).read()
     assert "RMHD_FLUX=split" in hdr and "test_ssp3_332_parity[blast_3d_split]" in hdr
+
+
+def test_release_staging_without_anything_to_release(B):
+    """No host-buffer batch call has run: nothing is held, nothing is touched (works without a GPU)."""
+    assert B.lib().rmhd_release_staging(-1) == B.RMHD_OK
+    assert B.lib().rmhd_release_staging(0) == B.RMHD_OK

@@ -530,6 +530,37 @@ def test_degenerate_calls(B, synth):
     assert ex.value.code == B.RMHD_ERR_BAD_PARAM
 
 
+def test_host_batches_reuse_one_staging_area(B, synth):
+    """Host-buffer batch calls stage through one grow-only device allocation (rmhd_release_staging, rmhd.h): a small call, a larger
+    one (the area grows), the small one again (stale contents of the larger call behind it), and once more after a release must all
+    give what the device-buffer path gives, bit for bit."""
+    import torch
+    def run(n, host):
+        c = synth.config2(n, seed=4)
+        P = B.make_params(**c["params"])
+        q_ex = np.empty((14, n)); B.rmhd_prim2cons_batch(P, c["prims"], q_ex)
+        if host:
+            q = np.empty_like(q_ex); w = np.empty_like(c["prims"]); it = np.zeros(n, np.int32); fl = np.zeros(n, np.int32)
+            B.rmhd_stage_batch(P, q_ex, c["prims"], c["a_dt"], q, w, c["sigma_cell"], it, fl)
+            w2 = np.empty_like(w); B.rmhd_con2prim_batch(P, q, w2, w)
+            return q, w, it, fl, w2
+        d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+        q = torch.empty(14, n, dtype=torch.float64, device="cuda"); w = torch.empty(11, n, dtype=torch.float64, device="cuda")
+        it = torch.zeros(n, dtype=torch.int32, device="cuda"); fl = torch.zeros(n, dtype=torch.int32, device="cuda")
+        B.rmhd_stage_batch(P, d(q_ex), d(c["prims"]), c["a_dt"], q, w, d(c["sigma_cell"]), it, fl)
+        w2 = torch.empty_like(w); B.rmhd_con2prim_batch(P, q, w2, w)
+        torch.cuda.synchronize()
+        return tuple(x.cpu().numpy() for x in (q, w, it, fl, w2))
+    ref = {n: run(n, host=False) for n in (1000, 70001)}
+    for n in (1000, 70001, 1000):
+        for a, b in zip(run(n, host=True), ref[n]):
+            assert np.array_equal(a, b, equal_nan=True)
+    B.rmhd_release_staging(0)
+    B.rmhd_release_staging(-1)          # nothing left: still fine
+    for a, b in zip(run(1000, host=True), ref[1000]):
+        assert np.array_equal(a, b, equal_nan=True)
+
+
 def test_set_cons_get_state_round_trip_and_device_buffers(B, O, synth):
     import torch
     c = synth.config3(nx=32, ny=24, nsteps=3)
