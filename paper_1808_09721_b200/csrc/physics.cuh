@@ -67,21 +67,34 @@ RMHD_DEV void hyd_from_Z(double D, double Sx, double Sy, double Sz, double S2, d
 // floor.  Taken automatically by c2p_hydro after C2P_SWITCH iterations of the first residual; never inlined (rare path).
 constexpr int C2P_SWITCH = 20;
 
+// primitives from a converged (or last) Lorentz factor W of the second residual; returns the c2p_hydro_W code
+RMHD_DEV int hyd_from_W(double D, double Sx, double Sy, double Sz, double En, double g, double W, bool conv, Hyd& h) {
+  const double Z = W * (En * W - g * D) / (W * W - g);
+  const double iZ = 1.0 / Z;
+  h.Z = Z; h.W = W;
+  h.p = g * (Z / (W * W) - D / W);
+  h.rho = D / W;
+  h.vx = Sx * iZ; h.vy = Sy * iZ; h.vz = Sz * iZ;
+  if (!conv) return 2;
+  if (!(h.p > 0.0) || !(h.rho > 0.0) || !isfinite(h.p) || !isfinite(Z)) return 3;
+  return 0;
+}
+
 __device__ __noinline__ int c2p_hydro_W(double D, double Sx, double Sy, double Sz, double S2, double taut, double g, double tol,
                                         int maxit, Hyd& h, int& iters) {
   const double Sabs = sqrt(S2), En = taut + D;
   double lo = 1.0, hi = rsqrt((En - Sabs) * (En + Sabs) / (En * En));
   const double floor_eps = 32.0 * 2.220446049250313e-16;
-  double W = hi;
-  bool conv = false;
   if (hi - 1.0 <= 1e-9) {
     // near-static state: W^2 - 1 carries only a few ulps of 1 (exactly 0 once |St| / En < 1e-8, where F(Wmax) would read
     // "no root"); the root in closed form, W = 1 + v^2 / 2 with v^2 = St^2 / Z(W = 1)^2, error O(v^4) <= 4e-18
     const double Z1 = (En - g * D) / (1.0 - g);
-    W = 1.0 + 0.5 * S2 / (Z1 * Z1);
     ++iters;
-    conv = true;
-  } else {
+    return hyd_from_W(D, Sx, Sy, Sz, En, g, 1.0 + 0.5 * S2 / (Z1 * Z1), true, h);
+  }
+  double W = hi;
+  bool conv = false;
+  {
     const double a = En * W - g * D, b = W * W - g, c = W * W - 1.0;
     const double t1 = a * a * c, t2 = S2 * b * b;
     if (!isfinite(hi) || !(t1 - t2 >= -floor_eps * (t1 + t2))) {
@@ -89,7 +102,7 @@ __device__ __noinline__ int c2p_hydro_W(double D, double Sx, double Sy, double S
       return 3;
     }
   }
-  while (!conv && iters < maxit) {
+  while (iters < maxit) {
     ++iters;
     const double a = En * W - g * D, b = W * W - g, c = W * W - 1.0;
     const double t1 = a * a * c, t2 = S2 * b * b;
@@ -103,15 +116,7 @@ __device__ __noinline__ int c2p_hydro_W(double D, double Sx, double Sy, double S
     W = Wn;
     if (fabs(dW) <= tol * W) { conv = true; break; }
   }
-  const double Z = W * (En * W - g * D) / (W * W - g);
-  const double iZ = 1.0 / Z;
-  h.Z = Z; h.W = W;
-  h.p = g * (Z / (W * W) - D / W);
-  h.rho = D / W;
-  h.vx = Sx * iZ; h.vy = Sy * iZ; h.vz = Sz * iZ;
-  if (!conv) return 2;
-  if (!(h.p > 0.0) || !(h.rho > 0.0) || !isfinite(h.p) || !isfinite(Z)) return 3;
-  return 0;
+  return hyd_from_W(D, Sx, Sy, Sz, En, g, W, conv, h);
 }
 
 RMHD_DEV int c2p_hydro(double D, double Sx, double Sy, double Sz, double taut, double Zg,
